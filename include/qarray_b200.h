@@ -1,0 +1,152 @@
+/*
+ * qarray_b200.h -- C ABI of the B200-native constant-capacitance-model ground-state search.
+ *
+ * The library implements ONE thing: the per-pixel ground-state charge search of arXiv 2404.04994 ("QArray") --
+ * continuous minimum -> integer candidates -> free energy -> argmin -- for open and closed quantum-dot arrays with the
+ * default, thresholded and brute-force candidate sets, as hand-written CUDA kernels for sm_100a.  "Lnnn" = line nnn of
+ * the paper text; R1..R12 = the readings listed in DESIGN.md.
+ *
+ * Notation (paper's): n_dot dots, n_gate gates, P gate-voltage vectors ("pixels"), c_dd the dot-dot Maxwell
+ * capacitance matrix (L35-L39 Eq. (2)), M = c_dd^-1 (L41), c_gd the positive gate->dot couplings, N_c = c_gd V_g
+ * (Eq. (6)), F the free energy (Eq. (4)), |e| = 1 (L486).
+ *
+ * Conventions
+ *   - "host" pointers are ordinary CPU memory; "device" pointers are CUDA global memory of the model's device.
+ *   - All matrices are row-major fp64.  V_g is [P, n_gate]; N is [P, n_dot] int32; E is [P] fp64 (L454 output shape).
+ *   - Output and workspace buffers are allocated and owned by the caller; the library never frees them.
+ *   - qa_ground_state_open / _closed are ASYNCHRONOUS on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream): they only enqueue kernels, never synchronise and never allocate.
+ *   - A qa_model is immutable after qa_model_set_sensor_dots and may be used by concurrent calls on different streams
+ *     (each call needs its own workspace).
+ *   - Errors are returned as qa_status; nothing throws or aborts.  There is no CPU fallback: without a CUDA device every
+ *     entry point that needs one returns QA_ERR_CUDA.
+ */
+#ifndef QARRAY_B200_H
+#define QARRAY_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define QA_API __attribute__((visibility("default")))
+#else
+#define QA_API
+#endif
+
+typedef struct qa_model qa_model; /* opaque, library-owned */
+
+typedef enum {
+    QA_OK = 0,
+    QA_ERR_INVALID_ARG = 1,      /* NULL pointer, P < 0, t outside [0,1], n_max < 0, workspace too small, ...          */
+    QA_ERR_NOT_SYMMETRIC = 2,    /* |C_ij - C_ji| > 1e-12 max|C|                                              (L204)   */
+    QA_ERR_NOT_POSDEF = 3,       /* Cholesky of c_dd fails                                                    (L204)   */
+    QA_ERR_UNSUPPORTED_SIZE = 4, /* n_dot > 16 or n_gate > 64                                                          */
+    QA_ERR_INFEASIBLE = 5,       /* closed array: N_hat < 0, or brute force with n_dot * n_max < N_hat                 */
+    QA_ERR_OVERFLOW = 6,         /* brute force: (n_max + 1)^n_dot >= 2^62                                             */
+    QA_ERR_CUDA = 7,             /* a CUDA runtime call failed; see qa_last_cuda_error()                               */
+    QA_ERR_UNSUPPORTED = 8       /* c_dd has a positive off-diagonal entry (not a Maxwell matrix, L35): the exact
+                                    clamp-only QP of reading R3 needs offdiag <= 0                                     */
+} qa_status;
+
+/* The three candidate sets of the paper (Table I). */
+typedef enum {
+    QA_ALG_DEFAULT = 0,     /* all 2^n_dot floor/ceil roundings of the continuous minimum           (L123-L127)        */
+    QA_ALG_THRESHOLDED = 1, /* both roundings only where |frac - 1/2| <= t/2, Eq. (9)               (L131-L141)        */
+    QA_ALG_BRUTE_FORCE = 2  /* every N in {0..n_max}^n_dot                                          (L13)              */
+} qa_algorithm;
+
+/* Optional per-call counters, accumulated on the device with atomics (zero the struct before the call). */
+typedef struct {
+    int64_t n_pixels;
+    int64_t n_qp_pixels;             /* pixels whose analytic minimum had a negative component (L82-L84, L106)         */
+    int64_t n_qp_rounds;             /* total active-set rounds over those pixels                                      */
+    int64_t n_candidates_enumerated; /* sum over pixels of the size of the enumerated set                              */
+    int64_t n_candidates_scored;     /* ... of those whose energy entered the argmin (closed: sum N = N_hat)           */
+    int64_t n_threshold_doublings;   /* closed + thresholded: times t was doubled (L141, reading R5)                   */
+    int64_t n_widened_pixels;        /* closed: floor/ceil set empty even at t = 1, set widened (reading R5)           */
+    int64_t n_qp_failed;             /* pixels whose QP did not reach a KKT point (must be 0)                          */
+} qa_stats;
+
+/* ---- model ------------------------------------------------------------------------------------------------------- */
+
+/* Problem statement: the constructor of the paper's DotArray (L185-L201) with Maxwell-format inputs.
+ * C_dd : host, [n_dot*n_dot], symmetric positive definite, off-diagonals <= 0 (L35, Eq. (B1)).  Validated as in
+ *        L204: finite, symmetric (QA_ERR_NOT_SYMMETRIC), positive definite (QA_ERR_NOT_POSDEF).
+ * C_gd : host, [n_dot*n_gate], gate->dot couplings (positive convention, reading on L35 vs L90).
+ * Computes M = c_dd^-1, c_dd 1, 1^T c_dd 1 (Eq. (7)) and the pixel-independent pair-energy tables on the host, and
+ * uploads them to the CURRENT CUDA device.  *out is owned by the library until qa_model_destroy. */
+QA_API qa_status qa_model_create(const double *C_dd, const double *C_gd, int n_dot, int n_gate, qa_model **out);
+
+/* Charge-sensor dots (L149, reading R8): the search runs on the sub-blocks C_dd[D,D], C_gd[D,:] of the non-sensor dots
+ * D; then each sensor dot's carrier number and potential V_s = [M (N - N_c)]_s (Eq. (3)) are computed in the full
+ * model.  dot_idx: host, n_sensor distinct indices in [0, n_dot); n_sensor = 0 clears.  Must be called before the model
+ * is used by any ground-state call still in flight. */
+QA_API qa_status qa_model_set_sensor_dots(qa_model *model, const int *dot_idx, int n_sensor);
+
+QA_API qa_status qa_model_destroy(qa_model *model);
+
+QA_API int qa_model_n_dot(const qa_model *model);    /* dots of the full model                                   */
+QA_API int qa_model_n_gate(const qa_model *model);
+QA_API int qa_model_n_sensor(const qa_model *model);
+QA_API int qa_model_n_search(const qa_model *model); /* n_dot - n_sensor: columns of d_xcont                     */
+/* M = c_dd^-1 of the full model as the library computed it (host, [n_dot*n_dot]) and E_C = 1/2 min_i M_ii. */
+QA_API qa_status qa_model_get_inverse(const qa_model *model, double *M_host, double *E_C);
+
+/* ---- ground state ------------------------------------------------------------------------------------------------ */
+
+/* Bytes of device scratch a call on P pixels needs (0 on invalid arguments).  The buffer must be 256-byte aligned. */
+QA_API size_t qa_workspace_bytes(const qa_model *model, int64_t P);
+
+/* Open array: constraints (i) integer, (ii) N_i >= 0 (L49-L52).  Paper API: ground_state_open(vg) (L454-L458).
+ *   d_Vg        device [P*n_gate]      gate voltages
+ *   alg, t      candidate set; t in [0,1] is read for QA_ALG_THRESHOLDED only (Eq. (9))
+ *   n_max       read for QA_ALG_BRUTE_FORCE only (L13)
+ *   d_N         device [P*n_dot] int32 ground-state charges N* (Eq. (5)); sensor dots in their own columns
+ *   d_E         device [P]             E(N*) = 1/2 (N*-N_c)^T M (N*-N_c) of the searched (sub-)model, recomputed from
+ *                                      the definition (Eq. (C1)); equals Eq. (4) + 1/2 N_c^T M N_c (reading R2)
+ *   d_xcont     device [P*n_search] or NULL   continuous minimum (Eq. (6)/(7)/(8))
+ *   d_Vsensor   device [P*n_sensor] or NULL   sensor-dot potentials (only for models with sensor dots)
+ *   d_stats     device qa_stats or NULL
+ *   d_workspace device, >= qa_workspace_bytes(model, P) bytes, 256-byte aligned; contents undefined afterwards
+ * Returns QA_OK once the work is enqueued. */
+QA_API qa_status qa_ground_state_open(const qa_model *model, const double *d_Vg, int64_t P, qa_algorithm alg, double t,
+                               int n_max, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor,
+                               qa_stats *d_stats, void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Closed array: additionally (iii) sum_i N_i = N_hat (L54-L56).  Paper API: ground_state_closed(vg, n_charges) (L454).
+ * Candidates with the wrong total are eliminated (L127, L159); thresholded: per-pixel threshold doubling (L141, R5). */
+QA_API qa_status qa_ground_state_closed(const qa_model *model, const double *d_Vg, int64_t P, int N_hat, qa_algorithm alg,
+                                 double t, int n_max, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor,
+                                 qa_stats *d_stats, void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Host-buffer convenience (the end-to-end path): same semantics with HOST pointers.  Copies V_g to the device, runs the
+ * search, copies the results back and synchronises before returning.  Device scratch comes from the stream-ordered pool
+ * (cudaMallocAsync) and is released before return.  closed = 0/1; N_hat is ignored for open arrays.  h_stats may be
+ * NULL; it is overwritten, not accumulated. */
+QA_API qa_status qa_ground_state_host(const qa_model *model, const double *h_Vg, int64_t P, int closed, int N_hat,
+                               qa_algorithm alg, double t, int n_max, int32_t *h_N, double *h_E, double *h_xcont,
+                               double *h_Vsensor, qa_stats *h_stats);
+
+/* ---- measurement aids -------------------------------------------------------------------------------------------- */
+
+/* Sustained FP64 issue rate of the current device: independent DFMA chains on every SM for about `seconds`.
+ * Returns FP64 thread-instructions per second (1 DFMA = 1) -- the denominator of the ALU roofline. */
+QA_API qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *cuda_stream);
+
+/* Names of the kernels the last ground-state call on this host thread enqueued (comma separated; static storage). */
+QA_API const char *qa_last_launch_plan(void);
+/* Number of kernels the last ground-state call on this host thread enqueued. */
+QA_API int qa_last_launch_count(void);
+
+QA_API const char *qa_status_string(qa_status s);
+QA_API const char *qa_last_cuda_error(void);
+QA_API const char *qa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QARRAY_B200_H */

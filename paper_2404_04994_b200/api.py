@@ -1,0 +1,234 @@
+"""Thin Python binding over the C ABI of libqarray_b200.so (include/qarray_b200.h): same names, argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device memory, streams and nothing
+else.  There is no CPU fallback: importing this module fails if the library is not built, and every ground-state call
+fails if there is no CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqarray_b200.so")
+
+QA_OK = 0
+QA_ALG_DEFAULT, QA_ALG_THRESHOLDED, QA_ALG_BRUTE_FORCE = 0, 1, 2
+ALG = {"default": 0, "thresholded": 1, "brute": 2, "brute_force": 2}
+STATUS_NAMES = ["QA_OK", "QA_ERR_INVALID_ARG", "QA_ERR_NOT_SYMMETRIC", "QA_ERR_NOT_POSDEF", "QA_ERR_UNSUPPORTED_SIZE",
+                "QA_ERR_INFEASIBLE", "QA_ERR_OVERFLOW", "QA_ERR_CUDA", "QA_ERR_UNSUPPORTED"]
+EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "qa_model_n_dot", "qa_model_n_gate",
+           "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
+           "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_last_launch_plan",
+           "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
+
+
+class qa_stats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("n_pixels", "n_qp_pixels", "n_qp_rounds", "n_candidates_enumerated",
+                                         "n_candidates_scored", "n_threshold_doublings", "n_widened_pixels",
+                                         "n_qp_failed")]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+class QaError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        msg = lib().qa_status_string(status).decode()
+        extra = lib().qa_last_cuda_error().decode() if status == 7 else ""
+        super().__init__(f"{where}: {name} ({msg}) {extra}".strip())
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """The loaded library; raises if it has not been built (python -m paper_2404_04994_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2404_04994_b200.build` "
+                              "(there is no CPU fallback)")
+        l = C.CDLL(LIB_PATH)
+        vp, dp, ip = C.c_void_p, C.c_void_p, C.c_void_p
+        l.qa_model_create.argtypes = [vp, vp, C.c_int, C.c_int, C.POINTER(vp)]
+        l.qa_model_set_sensor_dots.argtypes = [vp, vp, C.c_int]
+        l.qa_model_destroy.argtypes = [vp]
+        for f in ("qa_model_n_dot", "qa_model_n_gate", "qa_model_n_sensor", "qa_model_n_search"):
+            getattr(l, f).argtypes = [vp]
+        l.qa_model_get_inverse.argtypes = [vp, vp, C.POINTER(C.c_double)]
+        l.qa_workspace_bytes.argtypes = [vp, C.c_int64]
+        l.qa_workspace_bytes.restype = C.c_size_t
+        l.qa_ground_state_open.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp, vp, vp,
+                                           C.c_size_t, vp]
+        l.qa_ground_state_closed.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp, vp,
+                                             vp, C.c_size_t, vp]
+        l.qa_ground_state_host.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, vp, vp, vp,
+                                           vp, vp]
+        l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
+        l.qa_last_launch_plan.restype = C.c_char_p
+        l.qa_status_string.restype = C.c_char_p
+        l.qa_status_string.argtypes = [C.c_int]
+        l.qa_last_cuda_error.restype = C.c_char_p
+        l.qa_version.restype = C.c_char_p
+        _lib = l
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != QA_OK:
+        raise QaError(status, where)
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class Model:
+    """qa_model_create(C_dd, C_gd).  Owns the opaque handle."""
+
+    def __init__(self, C_dd, C_gd, sensor_dots=()):
+        C_dd = np.ascontiguousarray(C_dd, dtype=np.float64)
+        C_gd = np.ascontiguousarray(C_gd, dtype=np.float64)
+        if C_dd.ndim != 2 or C_dd.shape[0] != C_dd.shape[1] or C_gd.ndim != 2 or C_gd.shape[0] != C_dd.shape[0]:
+            raise QaError(1, "qa_model_create")
+        self._h = C.c_void_p()
+        _check(lib().qa_model_create(C_dd.ctypes.data, C_gd.ctypes.data, C_dd.shape[0], C_gd.shape[1],
+                                     C.byref(self._h)), "qa_model_create")
+        if len(sensor_dots):
+            self.set_sensor_dots(sensor_dots)
+        self._ws = None
+        self._stats = None
+
+    def set_sensor_dots(self, dots):
+        idx = np.ascontiguousarray(dots, dtype=np.int32)
+        _check(lib().qa_model_set_sensor_dots(self._h, idx.ctypes.data, len(idx)), "qa_model_set_sensor_dots")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().qa_model_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    n_dot = property(lambda self: lib().qa_model_n_dot(self._h))
+    n_gate = property(lambda self: lib().qa_model_n_gate(self._h))
+    n_sensor = property(lambda self: lib().qa_model_n_sensor(self._h))
+    n_search = property(lambda self: lib().qa_model_n_search(self._h))
+
+    def inverse(self):
+        M = np.empty((self.n_dot, self.n_dot))
+        ec = C.c_double()
+        _check(lib().qa_model_get_inverse(self._h, M.ctypes.data, C.byref(ec)), "qa_model_get_inverse")
+        return M, ec.value
+
+    def workspace_bytes(self, P: int) -> int:
+        return int(lib().qa_workspace_bytes(self._h, int(P)))
+
+    def _workspace(self, P, device):
+        need = self.workspace_bytes(P)
+        if self._ws is None or self._ws.numel() < need or self._ws.device != device:
+            self._ws = torch.empty(need, dtype=torch.uint8, device=device)
+        return self._ws
+
+    # -- device-resident call: the C-ABI entry points proper -----------------------------------------------------
+    def ground_state(self, Vg: torch.Tensor, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0,
+                     want_xcont=False, want_stats=False, out=None, stream=None):
+        """qa_ground_state_open / qa_ground_state_closed on a CUDA tensor Vg[P, n_gate] (float64).  Asynchronous on the
+        current torch stream.  Returns dict(N, E[, xcont][, Vsensor][, stats (a device tensor of 8 int64)])."""
+        if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
+            raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        Vg = Vg.contiguous().view(-1, self.n_gate)
+        P, dev = Vg.shape[0], Vg.device
+        out = out or {}
+        N = out.get("N")
+        if N is None:
+            N = torch.empty((P, self.n_dot), dtype=torch.int32, device=dev)
+        E = out.get("E")
+        if E is None:
+            E = torch.empty(P, dtype=torch.float64, device=dev)
+        xc = (out.get("xcont") if out.get("xcont") is not None
+              else torch.empty((P, self.n_search), dtype=torch.float64, device=dev)) if want_xcont else None
+        Vs = (out.get("Vsensor") if out.get("Vsensor") is not None
+              else torch.empty((P, self.n_sensor), dtype=torch.float64, device=dev)) if self.n_sensor else None
+        st = torch.zeros(8, dtype=torch.int64, device=dev) if want_stats else None
+        ws = self._workspace(P, dev)
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        sp = C.c_void_p(s.cuda_stream)
+        alg = ALG[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        if regime == "open":
+            rc = lib().qa_ground_state_open(self._h, _ptr(Vg), P, alg, float(t), int(n_max), _ptr(N), _ptr(E), _ptr(xc),
+                                            _ptr(Vs), _ptr(st), _ptr(ws), ws.numel(), sp)
+        elif regime == "closed":
+            rc = lib().qa_ground_state_closed(self._h, _ptr(Vg), P, int(N_hat), alg, float(t), int(n_max), _ptr(N),
+                                              _ptr(E), _ptr(xc), _ptr(Vs), _ptr(st), _ptr(ws), ws.numel(), sp)
+        else:
+            raise ValueError("regime must be 'open' or 'closed'")
+        _check(rc, f"qa_ground_state_{regime}")
+        res = {"N": N, "E": E}
+        if xc is not None:
+            res["xcont"] = xc
+        if Vs is not None:
+            res["Vsensor"] = Vs
+        if st is not None:
+            res["stats"] = st
+        return res
+
+    # -- host-buffer call (end-to-end path) -------------------------------------------------------------------------
+    def ground_state_host(self, Vg, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0, want_xcont=False,
+                          want_stats=False, out=None):
+        """qa_ground_state_host on HOST buffers (numpy arrays or CPU torch tensors, ideally pinned): H2D copy, search,
+        D2H copy and synchronisation all happen inside the C call."""
+        tv = Vg if isinstance(Vg, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(Vg, dtype=np.float64))
+        tv = tv.contiguous().view(-1, self.n_gate)
+        assert tv.dtype == torch.float64 and not tv.is_cuda
+        P = tv.shape[0]
+        out = out or {}
+        N = out.get("N") if out.get("N") is not None else torch.empty((P, self.n_dot), dtype=torch.int32)
+        E = out.get("E") if out.get("E") is not None else torch.empty(P, dtype=torch.float64)
+        xc = torch.empty((P, self.n_search), dtype=torch.float64) if want_xcont else None
+        Vs = torch.empty((P, self.n_sensor), dtype=torch.float64) if self.n_sensor else None
+        st = qa_stats() if want_stats else None
+        alg = ALG[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        rc = lib().qa_ground_state_host(self._h, _ptr(tv), P, int(regime == "closed"), int(N_hat), alg, float(t),
+                                        int(n_max), _ptr(N), _ptr(E), _ptr(xc), _ptr(Vs),
+                                        C.byref(st) if st is not None else None)
+        _check(rc, "qa_ground_state_host")
+        res = {"N": N, "E": E}
+        if xc is not None:
+            res["xcont"] = xc
+        if Vs is not None:
+            res["Vsensor"] = Vs
+        if st is not None:
+            res["stats"] = st.as_dict()
+        return res
+
+
+def stats_dict(t: torch.Tensor) -> dict:
+    v = t.cpu().tolist()
+    return {k: int(v[i]) for i, (k, _) in enumerate(qa_stats._fields_)}
+
+
+def measure_fp64_rate(seconds: float = 1.0) -> float:
+    """qa_measure_fp64_rate: sustained FP64 thread-instructions/s of the current device."""
+    r = C.c_double()
+    _check(lib().qa_measure_fp64_rate(float(seconds), C.byref(r), C.c_void_p(torch.cuda.current_stream().cuda_stream)),
+           "qa_measure_fp64_rate")
+    return r.value
+
+
+def last_launch_plan():
+    return lib().qa_last_launch_plan().decode().split(","), int(lib().qa_last_launch_count())
+
+
+def version() -> str:
+    return lib().qa_version().decode()

@@ -1,0 +1,437 @@
+// qa_api.cu -- host side of the C ABI (include/qarray_b200.h): model validation and setup (S0), argument checks,
+// workspace carving and kernel dispatch.  No compute on the host beyond S0; no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "qa_internal.cuh"
+
+struct qa_model {
+    int nf, g, ns;          // full model
+    int device;
+    int sm_count;
+    bool is_z;              // every off-diagonal of c_dd <= 0 (Maxwell, Eq. (B1))
+    double Cf[QA_MAXN * QA_MAXN];    // full c_dd, stride nf
+    double Cgdf[QA_MAXN * QA_MAXG];  // full c_gd, stride g
+    double Mf[QA_MAXN * QA_MAXN];    // full inverse, stride nf
+    double ECf;
+    int sens[QA_MAXN];
+    QaDevModel host;        // mirror of the device constants
+    QaDevModel *dev;        // device copy
+    QaWalkTable walk;       // pair table of the low bits of the search model
+};
+
+namespace {
+
+thread_local std::string g_plan;
+thread_local int g_plan_count = 0;
+thread_local char g_cuda_err[256] = "";
+
+qa_status cuda_fail(cudaError_t e, const char *where)
+{
+    std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return QA_ERR_CUDA;
+}
+#define QA_CUDA(call)                                                                                                  \
+    do {                                                                                                               \
+        cudaError_t e__ = (call);                                                                                      \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);                                                          \
+    } while (0)
+
+// Cholesky-based inverse of an SPD matrix (k x k, row-major, stride k).  Returns false if not positive definite.
+bool spd_inverse(const double *A, int k, double *inv)
+{
+    double L[QA_MAXN * QA_MAXN];
+    for (int i = 0; i < k; ++i) {
+        for (int j = 0; j <= i; ++j) {
+            double s = A[i * k + j];
+            for (int q = 0; q < j; ++q) s -= L[i * k + q] * L[j * k + q];
+            if (i == j) {
+                if (!(s > 0.0) || !std::isfinite(s)) return false;
+                L[i * k + i] = std::sqrt(s);
+            } else {
+                L[i * k + j] = s / L[j * k + j];
+            }
+        }
+    }
+    for (int c = 0; c < k; ++c) {
+        double y[QA_MAXN], x[QA_MAXN];
+        for (int i = 0; i < k; ++i) {
+            double s = (i == c) ? 1.0 : 0.0;
+            for (int q = 0; q < i; ++q) s -= L[i * k + q] * y[q];
+            y[i] = s / L[i * k + i];
+        }
+        for (int i = k - 1; i >= 0; --i) {
+            double s = y[i];
+            for (int q = i + 1; q < k; ++q) s -= L[q * k + i] * x[q];
+            x[i] = s / L[i * k + i];
+        }
+        for (int i = 0; i < k; ++i) inv[i * k + c] = x[i];
+    }
+    return true;
+}
+
+// (Re)build the search model (full model minus sensor dots), its tables, and upload.
+qa_status rebuild(qa_model *m)
+{
+    QaDevModel &h = m->host;
+    std::memset(&h, 0, sizeof(h));
+    const int nf = m->nf, g = m->g, ns = m->ns;
+    bool is_s[QA_MAXN] = {false};
+    for (int a = 0; a < ns; ++a) is_s[m->sens[a]] = true;
+    int n = 0;
+    for (int i = 0; i < nf; ++i)
+        if (!is_s[i]) h.arr_idx[n++] = i;
+    for (int a = 0; a < ns; ++a) h.sens_idx[a] = m->sens[a];
+    h.n = n;
+    h.g = g;
+    h.nf = nf;
+    h.ns = ns;
+    double Csub[QA_MAXN * QA_MAXN], Msub[QA_MAXN * QA_MAXN];
+    for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b) Csub[a * n + b] = m->Cf[h.arr_idx[a] * nf + h.arr_idx[b]];
+    if (!spd_inverse(Csub, n, Msub)) return QA_ERR_NOT_POSDEF;
+    double tot = 0.0, mn = 0.0;
+    for (int a = 0; a < n; ++a) {
+        double s = 0.0;  // c_dd 1: plain left-to-right sum (reading R1)
+        for (int b = 0; b < n; ++b) {
+            h.C[a * QA_MAXN + b] = Csub[a * n + b];
+            h.M[a * QA_MAXN + b] = Msub[a * n + b];
+            s = s + Csub[a * n + b];
+        }
+        h.C1[a] = s;
+        tot = tot + s;
+        for (int k = 0; k < g; ++k) h.Cgd[a * QA_MAXG + k] = m->Cgdf[h.arr_idx[a] * g + k];
+        if (a == 0 || Msub[a * n + a] < mn) mn = Msub[a * n + a];
+    }
+    h.oneC1 = tot;
+    h.EC = 0.5 * mn;
+    for (int i = 0; i < nf; ++i) {
+        for (int j = 0; j < nf; ++j) h.Mf[i * QA_MAXN + j] = m->Mf[i * nf + j];
+        for (int k = 0; k < g; ++k) h.Cgdf[i * QA_MAXG + k] = m->Cgdf[i * g + k];
+    }
+    // pair table of the low bits: low bit j <-> search dot n-1-j
+    const int nl = n < QA_WALK_NL ? n : QA_WALK_NL;
+    for (int b = 0; b < (1 << QA_WALK_NL); ++b) {
+        double s = 0.0;
+        if (b < (1 << nl))
+            for (int j = 0; j < nl; ++j)
+                for (int j2 = j + 1; j2 < nl; ++j2)
+                    if (((b >> j) & 1) && ((b >> j2) & 1)) s += Msub[(n - 1 - j) * n + (n - 1 - j2)];
+        m->walk.QL[b] = s;
+    }
+    QA_CUDA(cudaMemcpy(m->dev, &h, sizeof(h), cudaMemcpyHostToDevice));
+    return QA_OK;
+}
+
+size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
+{
+    const size_t n = (size_t)m->host.n, Pz = (size_t)P;
+    char *p = static_cast<char *>(base);
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        void *r = p ? p + off : nullptr;
+        off += align256(bytes);
+        return r;
+    };
+    double *h = static_cast<double *>(take(n * Pz * 8));
+    double *nc = static_cast<double *>(take(n * Pz * 8));
+    int32_t *bs = static_cast<int32_t *>(take(n * Pz * 4));
+    int32_t *ct = static_cast<int32_t *>(take(n * Pz * 4));
+    uint64_t *tt = static_cast<uint64_t *>(take(Pz * 8));
+    uint64_t *be = static_cast<uint64_t *>(take(Pz * 8));
+    if (ws) {
+        ws->h = h;
+        ws->nc = nc;
+        ws->base = bs;
+        ws->cnt = ct;
+        ws->total = tt;
+        ws->best = be;
+        ws->P = P;
+    }
+    return off;
+}
+
+qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int closed, int N_hat, qa_algorithm alg,
+                       double t, int n_max, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor,
+                       qa_stats *d_stats, void *d_ws, size_t ws_bytes, void *stream_v)
+{
+    qa_plan_reset();
+    if (!m || P < 0 || (P > 0 && (!d_Vg || !d_N || !d_E))) return QA_ERR_INVALID_ARG;
+    if (alg != QA_ALG_DEFAULT && alg != QA_ALG_THRESHOLDED && alg != QA_ALG_BRUTE_FORCE) return QA_ERR_INVALID_ARG;
+    if (alg == QA_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return QA_ERR_INVALID_ARG;
+    if (alg == QA_ALG_BRUTE_FORCE && n_max < 0) return QA_ERR_INVALID_ARG;
+    const int n = m->host.n;
+    if (closed && N_hat < 0) return QA_ERR_INFEASIBLE;
+    if (alg == QA_ALG_BRUTE_FORCE) {
+        if (std::pow((double)n_max + 1.0, (double)n) >= 4.611686018427388e18) return QA_ERR_OVERFLOW;
+        if (closed && (int64_t)n * n_max < N_hat) return QA_ERR_INFEASIBLE;
+    }
+    if (!m->is_z) return QA_ERR_UNSUPPORTED;
+    if (P == 0) return QA_OK;
+    if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
+    if (!d_ws || ws_bytes < carve(m, P, nullptr, nullptr) || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
+        return QA_ERR_INVALID_ARG;
+    QaWorkspace ws;
+    carve(m, P, d_ws, &ws);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max};
+    QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
+    if (alg == QA_ALG_DEFAULT && !closed) {
+        QA_CUDA(qa_launch_walk(m->dev, n, m->walk, ws, d_stats, m->sm_count, stream));
+    } else {
+        double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n)
+                        : alg == QA_ALG_DEFAULT   ? std::pow(2.0, (double)n)
+                                                  : std::pow(1.0 + t, (double)n);
+        QA_CUDA(qa_launch_enumerate(m->dev, n, ws, a, expect, d_stats, stream));
+    }
+    QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream));
+    return QA_OK;
+}
+
+}  // namespace
+
+void qa_plan_reset()
+{
+    g_plan.clear();
+    g_plan_count = 0;
+}
+void qa_plan_add(const char *name)
+{
+    if (!g_plan.empty()) g_plan += ",";
+    g_plan += name;
+    ++g_plan_count;
+}
+
+extern "C" {
+
+qa_status qa_model_create(const double *C_dd, const double *C_gd, int n_dot, int n_gate, qa_model **out)
+{
+    if (out) *out = nullptr;
+    if (!C_dd || !C_gd || !out || n_dot < 1 || n_gate < 1) return QA_ERR_INVALID_ARG;
+    if (n_dot > QA_MAXN || n_gate > QA_MAXG) return QA_ERR_UNSUPPORTED_SIZE;
+    double amax = 0.0;
+    for (int i = 0; i < n_dot * n_dot; ++i) {
+        if (!std::isfinite(C_dd[i])) return QA_ERR_INVALID_ARG;
+        amax = std::fmax(amax, std::fabs(C_dd[i]));
+    }
+    for (int i = 0; i < n_dot * n_gate; ++i)
+        if (!std::isfinite(C_gd[i])) return QA_ERR_INVALID_ARG;
+    bool is_z = true;
+    for (int i = 0; i < n_dot; ++i)
+        for (int j = 0; j < i; ++j) {
+            if (std::fabs(C_dd[i * n_dot + j] - C_dd[j * n_dot + i]) > 1e-12 * amax) return QA_ERR_NOT_SYMMETRIC;
+            if (C_dd[i * n_dot + j] > 0.0) is_z = false;
+        }
+    qa_model *m = new (std::nothrow) qa_model;
+    if (!m) return QA_ERR_INVALID_ARG;
+    std::memset(static_cast<void *>(m), 0, sizeof(*m));
+    m->nf = n_dot;
+    m->g = n_gate;
+    m->ns = 0;
+    m->is_z = is_z;
+    std::memcpy(m->Cf, C_dd, sizeof(double) * n_dot * n_dot);
+    std::memcpy(m->Cgdf, C_gd, sizeof(double) * n_dot * n_gate);
+    if (!spd_inverse(m->Cf, n_dot, m->Mf)) {
+        delete m;
+        return QA_ERR_NOT_POSDEF;
+    }
+    double mn = m->Mf[0];
+    for (int i = 1; i < n_dot; ++i) mn = std::fmin(mn, m->Mf[i * n_dot + i]);
+    m->ECf = 0.5 * mn;
+    cudaError_t e = cudaGetDevice(&m->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, m->device);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&m->dev), sizeof(QaDevModel));
+    if (e != cudaSuccess) {
+        delete m;
+        return cuda_fail(e, "qa_model_create");
+    }
+    qa_status s = rebuild(m);
+    if (s != QA_OK) {
+        cudaFree(m->dev);
+        delete m;
+        return s;
+    }
+    *out = m;
+    return QA_OK;
+}
+
+qa_status qa_model_set_sensor_dots(qa_model *m, const int *dot_idx, int n_sensor)
+{
+    if (!m || n_sensor < 0 || n_sensor >= m->nf || (n_sensor > 0 && !dot_idx)) return QA_ERR_INVALID_ARG;
+    bool seen[QA_MAXN] = {false};
+    for (int a = 0; a < n_sensor; ++a) {
+        if (dot_idx[a] < 0 || dot_idx[a] >= m->nf || seen[dot_idx[a]]) return QA_ERR_INVALID_ARG;
+        seen[dot_idx[a]] = true;
+    }
+    int old_ns = m->ns, old[QA_MAXN];
+    std::memcpy(old, m->sens, sizeof(old));
+    m->ns = n_sensor;
+    for (int a = 0; a < n_sensor; ++a) m->sens[a] = dot_idx[a];
+    qa_status s = rebuild(m);
+    if (s != QA_OK) {
+        m->ns = old_ns;
+        std::memcpy(m->sens, old, sizeof(old));
+        rebuild(m);
+    }
+    return s;
+}
+
+qa_status qa_model_destroy(qa_model *m)
+{
+    if (!m) return QA_OK;
+    cudaError_t e = cudaFree(m->dev);
+    delete m;
+    return e == cudaSuccess ? QA_OK : cuda_fail(e, "qa_model_destroy");
+}
+
+int qa_model_n_dot(const qa_model *m) { return m ? m->nf : 0; }
+int qa_model_n_gate(const qa_model *m) { return m ? m->g : 0; }
+int qa_model_n_sensor(const qa_model *m) { return m ? m->ns : 0; }
+int qa_model_n_search(const qa_model *m) { return m ? m->host.n : 0; }
+
+qa_status qa_model_get_inverse(const qa_model *m, double *M_host, double *E_C)
+{
+    if (!m) return QA_ERR_INVALID_ARG;
+    if (M_host) std::memcpy(M_host, m->Mf, sizeof(double) * m->nf * m->nf);
+    if (E_C) *E_C = m->ECf;
+    return QA_OK;
+}
+
+size_t qa_workspace_bytes(const qa_model *m, int64_t P)
+{
+    if (!m || P < 0) return 0;
+    return carve(m, P < 1 ? 1 : P, nullptr, nullptr);
+}
+
+qa_status qa_ground_state_open(const qa_model *m, const double *d_Vg, int64_t P, qa_algorithm alg, double t, int n_max,
+                               int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor, qa_stats *d_stats,
+                               void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    return ground_state(m, d_Vg, P, 0, 0, alg, t, n_max, d_N, d_E, d_xcont, d_Vsensor, d_stats, d_workspace,
+                        workspace_bytes, cuda_stream);
+}
+
+qa_status qa_ground_state_closed(const qa_model *m, const double *d_Vg, int64_t P, int N_hat, qa_algorithm alg, double t,
+                                 int n_max, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor,
+                                 qa_stats *d_stats, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    return ground_state(m, d_Vg, P, 1, N_hat, alg, t, n_max, d_N, d_E, d_xcont, d_Vsensor, d_stats, d_workspace,
+                        workspace_bytes, cuda_stream);
+}
+
+qa_status qa_ground_state_host(const qa_model *m, const double *h_Vg, int64_t P, int closed, int N_hat, qa_algorithm alg,
+                               double t, int n_max, int32_t *h_N, double *h_E, double *h_xcont, double *h_Vsensor,
+                               qa_stats *h_stats)
+{
+    if (!m || P < 0 || (P > 0 && (!h_Vg || !h_N || !h_E))) return QA_ERR_INVALID_ARG;
+    if (P == 0) return QA_OK;
+    const size_t Pz = (size_t)P, nf = (size_t)m->nf, n = (size_t)m->host.n, g = (size_t)m->g, ns = (size_t)m->ns;
+    const size_t bVg = align256(Pz * g * 8), bN = align256(Pz * nf * 4), bE = align256(Pz * 8);
+    const size_t bX = h_xcont ? align256(Pz * n * 8) : 0, bVs = (h_Vsensor && ns) ? align256(Pz * ns * 8) : 0;
+    const size_t bS = h_stats ? align256(sizeof(qa_stats)) : 0, bW = qa_workspace_bytes(m, P);
+    cudaStream_t stream = nullptr;
+    char *buf = nullptr;
+    QA_CUDA(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
+    qa_status st = QA_OK;
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&buf), bVg + bN + bE + bX + bVs + bS + bW, stream);
+    if (e != cudaSuccess) {
+        cudaStreamDestroy(stream);
+        return cuda_fail(e, "cudaMallocAsync");
+    }
+    double *dVg = reinterpret_cast<double *>(buf);
+    int32_t *dN = reinterpret_cast<int32_t *>(buf + bVg);
+    double *dE = reinterpret_cast<double *>(buf + bVg + bN);
+    double *dX = bX ? reinterpret_cast<double *>(buf + bVg + bN + bE) : nullptr;
+    double *dVs = bVs ? reinterpret_cast<double *>(buf + bVg + bN + bE + bX) : nullptr;
+    qa_stats *dS = bS ? reinterpret_cast<qa_stats *>(buf + bVg + bN + bE + bX + bVs) : nullptr;
+    void *dW = buf + bVg + bN + bE + bX + bVs + bS;
+    e = cudaMemcpyAsync(dVg, h_Vg, Pz * g * 8, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess && dS) e = cudaMemsetAsync(dS, 0, sizeof(qa_stats), stream);
+    if (e == cudaSuccess) {
+        st = ground_state(m, dVg, P, closed, N_hat, alg, t, n_max, dN, dE, dX, dVs, dS, dW, bW, stream);
+        if (st == QA_OK) {
+            e = cudaMemcpyAsync(h_N, dN, Pz * nf * 4, cudaMemcpyDeviceToHost, stream);
+            if (e == cudaSuccess) e = cudaMemcpyAsync(h_E, dE, Pz * 8, cudaMemcpyDeviceToHost, stream);
+            if (e == cudaSuccess && dX) e = cudaMemcpyAsync(h_xcont, dX, Pz * n * 8, cudaMemcpyDeviceToHost, stream);
+            if (e == cudaSuccess && dVs)
+                e = cudaMemcpyAsync(h_Vsensor, dVs, Pz * ns * 8, cudaMemcpyDeviceToHost, stream);
+            if (e == cudaSuccess && dS)
+                e = cudaMemcpyAsync(h_stats, dS, sizeof(qa_stats), cudaMemcpyDeviceToHost, stream);
+        }
+    }
+    cudaFreeAsync(buf, stream);
+    cudaError_t e2 = cudaStreamSynchronize(stream);
+    cudaStreamDestroy(stream);
+    if (st != QA_OK) return st;
+    if (e != cudaSuccess) return cuda_fail(e, "qa_ground_state_host");
+    if (e2 != cudaSuccess) return cuda_fail(e2, "qa_ground_state_host sync");
+    return QA_OK;
+}
+
+qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *cuda_stream)
+{
+    if (!thread_inst_per_s || !(seconds > 0.0)) return QA_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, sms = 0;
+    QA_CUDA(cudaGetDevice(&dev));
+    QA_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double *sink = nullptr;
+    QA_CUDA(cudaMalloc(reinterpret_cast<void **>(&sink), 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int blocks = sms * 8, threads = 256;
+    int iters = 2000;
+    double rate = 0.0;
+    qa_status st = QA_OK;
+    for (int pass = 0; pass < 3 && st == QA_OK; ++pass) {  // warm-up / calibrate / measure
+        cudaEventRecord(e0, stream);
+        cudaError_t e = qa_launch_fp64_probe(sink, blocks, threads, iters, stream);
+        cudaEventRecord(e1, stream);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) {
+            st = cuda_fail(e, "qa_measure_fp64_rate");
+            break;
+        }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        rate = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
+        if (pass == 1 || pass == 0) {
+            double want = (pass == 0 ? 0.05 : seconds) / (ms * 1e-3) * iters;
+            iters = want > 2e9 ? 2000000000 : (want < 100 ? 100 : (int)want);
+        }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    *thread_inst_per_s = rate;
+    return st;
+}
+
+const char *qa_last_launch_plan(void) { return g_plan.c_str(); }
+int qa_last_launch_count(void) { return g_plan_count; }
+
+const char *qa_status_string(qa_status s)
+{
+    switch (s) {
+        case QA_OK: return "ok";
+        case QA_ERR_INVALID_ARG: return "invalid argument";
+        case QA_ERR_NOT_SYMMETRIC: return "c_dd is not symmetric";
+        case QA_ERR_NOT_POSDEF: return "c_dd is not positive definite";
+        case QA_ERR_UNSUPPORTED_SIZE: return "n_dot > 16 or n_gate > 64";
+        case QA_ERR_INFEASIBLE: return "closed array: no admissible charge state";
+        case QA_ERR_OVERFLOW: return "brute force: (n_max+1)^n_dot >= 2^62";
+        case QA_ERR_CUDA: return "CUDA error";
+        case QA_ERR_UNSUPPORTED: return "c_dd has a positive off-diagonal entry (not a Maxwell matrix)";
+    }
+    return "unknown status";
+}
+const char *qa_last_cuda_error(void) { return g_cuda_err; }
+const char *qa_version(void) { return "qarray_b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

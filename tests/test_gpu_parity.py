@@ -1,0 +1,236 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI binding, against the oracle, element by element on
+the same seeded inputs; plus edge cases and full-size sampled checks in the launch configuration bench.py times."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2404_04994_b200 import workloads as wl
+from parity import compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2404_04994_b200 import api as _api
+    assert torch.cuda.is_available()
+    return _api
+
+
+def run_gpu(api, w, **kw):
+    m = api.Model(w.C_dd, w.C_gd, sensor_dots=w.sensor_dots)
+    Vg = torch.from_numpy(w.Vg).cuda()
+    r = m.ground_state(Vg, regime=w.regime, N_hat=w.N_hat, want_xcont=True, want_stats=True, **kw)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy() for k, v in r.items() if k != "stats"}
+    out["stats"] = api.stats_dict(r["stats"])
+    out["plan"] = api.last_launch_plan()
+    M, EC = m.inverse()
+    out["EC"] = EC
+    return out
+
+
+def run_oracle(w, **kw):
+    m = oracle.Model(w.C_dd, w.C_gd)
+    kw = dict(kw)
+    if "algorithm" in kw and kw["algorithm"] == "brute_force":
+        kw["algorithm"] = "brute"
+    return m, m.ground_state(w.Vg, regime=w.regime, N_hat=w.N_hat, **kw)
+
+
+def check(api, w, **kw):
+    g = run_gpu(api, w, **kw)
+    m, o = run_oracle(w, **kw)
+    rep = compare(g["N"], g["E"], o, m.EC, gpu_x=g["xcont"])
+    st = g["stats"]
+    assert st["n_pixels"] == w.P and st["n_qp_failed"] == 0
+    assert st["n_qp_pixels"] == int(((o["flags"] & oracle.FLAG_QP) != 0).sum())
+    assert st["n_candidates_enumerated"] == int(o["n_enum"].sum())
+    assert st["n_candidates_scored"] == int(o["n_scored"].sum())
+    assert st["n_threshold_doublings"] == int(o["doublings"].sum())
+    assert st["n_widened_pixels"] == int(((o["flags"] & oracle.FLAG_WIDENED) != 0).sum())
+    assert abs(g["EC"] - m.EC) <= 1e-12 * m.EC
+    return rep, g, o
+
+
+# ---- the five BASELINE.json configs at sizes the oracle finishes in seconds (several tiles + ragged tails) ----------
+def test_config1_open_double_dot_default_and_brute(api):
+    w = wl.config1(100, 100)
+    rep, g, o = check(api, w, algorithm="default")
+    assert "qa_walk_kernel" in g["plan"][0]
+    assert st_zero_qp(g)
+    check(api, w, algorithm="brute", n_max=5)
+
+
+def st_zero_qp(g):
+    return g["stats"]["n_qp_pixels"] == 0
+
+
+def test_config2_closed_chain_default_and_brute(api):
+    w = wl.config2(100, 100)
+    rep, g, o = check(api, w, algorithm="default")
+    assert g["stats"]["n_qp_pixels"] > 0
+    assert (g["N"].sum(1) == 5).all()
+    w2 = wl.config2(37, 23)
+    check(api, w2, algorithm="brute", n_max=5)
+    check(api, w2, algorithm="thresholded", t=0.3)
+    check(api, w2, algorithm="thresholded", t=0.0)
+
+
+def test_config3_sensor(api):
+    w = wl.config3(64, 45)
+    g = run_gpu(api, w, algorithm="default")
+    o = oracle.sensor_ground_state(w.C_dd, w.C_gd, w.sensor_dots, w.Vg)
+    full = oracle.Model(w.C_dd, w.C_gd)
+    D = [0, 1, 2, 3]
+    sub = oracle.Model(w.C_dd[np.ix_(D, D)], w.C_gd[D, :])
+    rep = compare(g["N"], g["E"], o, sub.EC, cols=D)
+    same = (g["N"] == o["N"]).all(1)
+    assert same.mean() > 0.999
+    assert np.allclose(g["Vsensor"][same], o["Vs"][same], rtol=1e-9, atol=1e-9 * full.EC)
+    assert g["xcont"].shape == (w.P, 4)
+
+
+@pytest.mark.parametrize("W,H", [(9, 7), (33, 3)])
+def test_config4_open_grid16_default(api, W, H):
+    """n = 16, 2^16 candidates per pixel: the hot kernel (NL = 8, NH = 8), QP pixels included."""
+    w = wl.config4(W, H)
+    rep, g, o = check(api, w, algorithm="default")
+    assert g["plan"][0] == ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"]
+    assert g["stats"]["n_candidates_scored"] == w.P * 65536
+
+
+def test_config5_open_grid8_default_and_thresholded(api):
+    for j in (0, 7):
+        w = wl.config5_array(j, 48, 41)
+        check(api, w, algorithm="default")
+        for t in (0.2, 0.5, 1.0):
+            check(api, w, algorithm="thresholded", t=t)
+
+
+# ---- every n_dot through the static walk and the generic enumeration ----------------------------------------------
+@pytest.mark.parametrize("n", list(range(1, 13)))
+def test_all_sizes_default_open(api, n):
+    w = wl.random_open(n, n + (n % 3), 301 if n <= 10 else 67, seed=50 + n)
+    check(api, w, algorithm="default")
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 6, 9, 11])
+def test_all_sizes_closed_and_thresholded(api, n):
+    w = wl.random_open(n, n, 203, seed=80 + n, lo=-0.4, hi=2.5)
+    w.regime, w.N_hat = "closed", max(1, n)
+    check(api, w, algorithm="default")
+    check(api, w, algorithm="thresholded", t=0.25)
+    w.regime = "open"
+    check(api, w, algorithm="thresholded", t=0.4)
+    if n <= 6:
+        check(api, w, algorithm="brute", n_max=3)
+        w.regime = "closed"
+        check(api, w, algorithm="brute", n_max=3)
+
+
+# ---- edge cases -----------------------------------------------------------------------------------------------------
+def test_edge_cases(api):
+    w = wl.config1(4, 4)
+    m = api.Model(w.C_dd, w.C_gd)
+    # empty input
+    r = m.ground_state(torch.empty((0, 2), dtype=torch.float64, device="cuda"))
+    assert r["N"].shape == (0, 2)
+    # single pixel, all-negative N_c (everything clamped -> N = 0)
+    r = m.ground_state(torch.tensor([[-3.0, -2.0]], dtype=torch.float64, device="cuda"), want_xcont=True)
+    assert r["N"].cpu().tolist() == [[0, 0]] and r["xcont"].cpu().tolist() == [[0.0, 0.0]]
+    # closed with N_hat = 0
+    r = m.ground_state(torch.from_numpy(w.Vg).cuda(), regime="closed", N_hat=0)
+    assert int(r["N"].abs().sum()) == 0
+    # argument errors
+    with pytest.raises(api.QaError) as e:
+        m.ground_state(torch.from_numpy(w.Vg).cuda(), algorithm="thresholded", t=1.5)
+    assert e.value.status == 1
+    with pytest.raises(api.QaError) as e:
+        m.ground_state(torch.from_numpy(w.Vg).cuda(), regime="closed", N_hat=-1)
+    assert e.value.status == 5
+    with pytest.raises(api.QaError) as e:
+        m.ground_state(torch.from_numpy(w.Vg).cuda(), regime="closed", N_hat=30, algorithm="brute", n_max=3)
+    assert e.value.status == 5
+    w16 = wl.config4(2, 2)
+    m16 = api.Model(w16.C_dd, w16.C_gd)
+    with pytest.raises(api.QaError) as e:
+        m16.ground_state(torch.from_numpy(w16.Vg).cuda(), algorithm="brute", n_max=20)
+    assert e.value.status == 6
+    with pytest.raises(api.QaError) as e:
+        api.Model(np.array([[1.0, 0.3], [0.1, 1.0]]), np.eye(2))
+    assert e.value.status == 2
+    with pytest.raises(api.QaError) as e:
+        api.Model(np.array([[1.0, -3.0], [-3.0, 1.0]]), np.eye(2))
+    assert e.value.status == 3
+    with pytest.raises(api.QaError) as e:
+        api.Model(np.eye(17), np.eye(17))
+    assert e.value.status == 4
+    mp = api.Model(np.array([[1.0, 0.1], [0.1, 1.0]]), np.eye(2))
+    with pytest.raises(api.QaError) as e:
+        mp.ground_state(torch.from_numpy(w.Vg).cuda())
+    assert e.value.status == 8
+    with pytest.raises(TypeError):
+        m.ground_state(torch.from_numpy(w.Vg))          # no CPU path
+
+
+def test_host_entry_point_matches_device_entry_point(api):
+    w = wl.config2(40, 30)
+    m = api.Model(w.C_dd, w.C_gd)
+    a = m.ground_state(torch.from_numpy(w.Vg).cuda(), regime="closed", N_hat=5)
+    b = m.ground_state_host(torch.from_numpy(w.Vg).pin_memory(), regime="closed", N_hat=5, want_stats=True)
+    assert torch.equal(a["N"].cpu(), b["N"]) and torch.equal(a["E"].cpu(), b["E"])
+    assert b["stats"]["n_pixels"] == w.P
+
+
+def test_deterministic_across_runs_and_streams(api):
+    w = wl.config4(8, 8)
+    m = api.Model(w.C_dd, w.C_gd)
+    Vg = torch.from_numpy(w.Vg).cuda()
+    a = m.ground_state(Vg)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        m2 = api.Model(w.C_dd, w.C_gd)
+        b = m2.ground_state(Vg)
+    torch.cuda.synchronize()
+    assert torch.equal(a["N"], b["N"]) and torch.equal(a["E"], b["E"])
+
+
+# ---- full BASELINE.json sizes in bench.py's launch configuration: sampled outputs + properties ---------------------
+def test_full_size_config4_sampled(api):
+    w = wl.config4(100, 100)
+    m = api.Model(w.C_dd, w.C_gd)
+    r = m.ground_state(torch.from_numpy(w.Vg).cuda(), want_xcont=True)
+    N, E, x = r["N"].cpu().numpy(), r["E"].cpu().numpy(), r["xcont"].cpu().numpy()
+    assert (N >= 0).all() and (N - np.floor(x) >= 0).all() and (N - np.floor(x) <= 1).all()
+    rng = np.random.default_rng(0)
+    sel = np.sort(rng.choice(w.P, size=24, replace=False))
+    om = oracle.Model(w.C_dd, w.C_gd)
+    o = om.ground_state(w.Vg[sel])
+    compare(N[sel], E[sel], o, om.EC, gpu_x=x[sel])
+    # property at any size: E(N*) equals the definition, and no single-dot move inside the candidate box lowers it
+    Minv = np.linalg.inv(w.C_dd)
+    nc = w.Vg @ w.C_gd.T
+    d = N - nc
+    assert np.allclose(E, 0.5 * np.einsum("pi,ij,pj->p", d, Minv, d), rtol=1e-9)
+    grad = d @ Minv
+    lo = np.maximum(np.floor(x), 0)
+    up_ok = (N - lo) < 1
+    dn_ok = (N - lo) > 0
+    half = 0.5 * np.diag(Minv)
+    assert (np.where(up_ok, grad + half, 1.0) >= -1e-9).all()
+    assert (np.where(dn_ok, -grad + half, 1.0) >= -1e-9).all()
+
+
+def test_full_size_config5_batch_member_sampled(api):
+    w = wl.config5_array(3)
+    m = api.Model(w.C_dd, w.C_gd)
+    om = oracle.Model(w.C_dd, w.C_gd)
+    rng = np.random.default_rng(1)
+    sel = np.sort(rng.choice(w.P, size=3000, replace=False))
+    Vg = torch.from_numpy(w.Vg).cuda()
+    for kw in (dict(algorithm="default"), dict(algorithm="thresholded", t=0.2), dict(algorithm="thresholded", t=0.5)):
+        r = m.ground_state(Vg, **kw)
+        o = om.ground_state(w.Vg[sel], **kw)
+        compare(r["N"].cpu().numpy()[sel], r["E"].cpu().numpy()[sel], o, om.EC)

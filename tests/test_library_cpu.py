@@ -1,0 +1,121 @@
+"""CPU-side checks of the product: the C-ABI library loads and exports every symbol include/qarray_b200.h declares, the
+binding refuses to run without a device (no CPU fallback), host-side validation works without a GPU, and the N > 1
+pixel-range sharding is covered with a world_size-2 gloo run."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_functions():
+    src = open(os.path.join(ROOT, "include", "qarray_b200.h")).read()
+    return sorted(set(re.findall(r"QA_API[^;(]*?\b(qa_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_builds_loads_and_exports_every_declared_symbol():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2404_04994_b200 import api
+    lib = api.lib()
+    names = header_functions()
+    assert len(names) >= 18 and sorted(api.EXPORTS) == names
+    for n in names:
+        assert hasattr(lib, n), n
+    out = subprocess.run(["nm", "-D", "--defined-only", api.LIB_PATH], capture_output=True, text=True).stdout
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l)
+    assert exported == names, "the library must export exactly the C ABI"
+    assert b"sm_100a" in api.lib().qa_version()
+
+
+def test_sass_is_sm100a_only():
+    from paper_2404_04994_b200 import api
+    out = subprocess.run(["cuobjdump", "-lelf", api.LIB_PATH], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, archs
+
+
+def test_status_strings_and_host_side_validation_without_gpu():
+    from paper_2404_04994_b200 import api
+    lib = api.lib()
+    for s in range(9):
+        assert len(lib.qa_status_string(s)) > 0
+    h = C.c_void_p()
+    bad = np.array([[1.0, 0.5], [0.1, 1.0]])
+    assert lib.qa_model_create(bad.ctypes.data, np.eye(2).ctypes.data, 2, 2, C.byref(h)) == 2      # not symmetric
+    notpd = np.array([[1.0, -3.0], [-3.0, 1.0]])
+    assert lib.qa_model_create(notpd.ctypes.data, np.eye(2).ctypes.data, 2, 2, C.byref(h)) == 3    # not pos. def.
+    assert lib.qa_model_create(np.eye(17).ctypes.data, np.eye(17).ctypes.data, 17, 17, C.byref(h)) == 4
+    assert lib.qa_model_create(None, None, 2, 2, C.byref(h)) == 1
+    assert lib.qa_workspace_bytes(None, 10) == 0
+    if not torch.cuda.is_available():
+        ok = np.array([[1.3, -0.1], [-0.1, 1.3]])
+        assert lib.qa_model_create(ok.ctypes.data, np.eye(2).ctypes.data, 2, 2, C.byref(h)) == 7   # QA_ERR_CUDA, loud
+        assert len(lib.qa_last_cuda_error()) > 0
+
+
+def test_no_cpu_fallback_in_binding():
+    from paper_2404_04994_b200 import api
+    from paper_2404_04994_b200 import workloads as wl
+    w = wl.config1(4, 4)
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(api.QaError):
+        api.Model(w.C_dd, w.C_gd)
+    src = open(os.path.join(ROOT, "paper_2404_04994_b200", "api.py")).read()
+    assert "import oracle" not in src and "from oracle" not in src
+    for f in os.listdir(os.path.join(ROOT, "paper_2404_04994_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_2404_04994_b200", "csrc", f)).read().lower().replace(
+            "no cpu fallback", "")
+
+
+def test_shard_range_partitions_pixels():
+    from paper_2404_04994_b200.workloads import shard_range
+    for P in (0, 1, 7, 100, 10000):
+        for world in (1, 2, 3, 8):
+            r = [shard_range(P, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == P
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+            sizes = [b - a for a, b in r]
+            assert max(sizes) - min(sizes) <= 1
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch, torch.distributed as dist
+import oracle
+from paper_2404_04994_b200 import workloads as wl
+dist.init_process_group("gloo", rank=int(os.environ["RANK"]), world_size=int(os.environ["WORLD_SIZE"]))
+rank, world = dist.get_rank(), dist.get_world_size()
+w = wl.config2(20, 13)
+p0, p1 = wl.shard_range(w.P, rank, world)
+m = oracle.Model(w.C_dd, w.C_gd)          # stand-in compute for the CPU test; the sharding logic is what is tested
+part = m.ground_state(w.Vg[p0:p1], regime="closed", N_hat=5)["N"]
+sizes = [wl.shard_range(w.P, r, world) for r in range(world)]
+bufs = [torch.empty((b - a, w.n_dot), dtype=torch.int32) for a, b in sizes]
+dist.all_gather(bufs, torch.from_numpy(part))   # final gather of the int32 maps: no data-path collective before it
+full = torch.cat(bufs).numpy()
+ref = m.ground_state(w.Vg, regime="closed", N_hat=5)["N"]
+t = torch.tensor([float(p1 - p0)]); dist.all_reduce(t)
+assert int(t.item()) == w.P
+assert np.array_equal(full, ref)
+dist.barrier(); dist.destroy_process_group()
+print("rank", rank, "ok")
+"""
+
+
+def test_two_rank_gloo_pixel_sharding(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29561", WORLD_SIZE="2")
+    procs = [subprocess.Popen([sys.executable, str(script)], env=dict(env, RANK=str(r)), stdout=subprocess.PIPE,
+                              stderr=subprocess.STDOUT, text=True) for r in range(2)]
+    outs = [p.communicate(timeout=240)[0] for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
