@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ground-state charge search on the headline workload (BASELINE.json configs[3]:
+open 4x4 grid of 16 dots, default algorithm, 100x100 pixels, 2^16 candidates per pixel, fp64).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config5]
+
+One "step" = one pass of the whole hot path (prologue -> candidate walk -> finalize) over
+one 100x100 diagram.  Prints ONE JSON line (rank 0).  Multi-GPU: one process per GPU (torchrun), every rank runs its own
+diagram (pixels are independent: no data-path collective), value = total candidates / max-over-ranks time ("weak").
+
+--impl reference times the ORACLE (oracle/, plain single-threaded C written from the paper) on the host cores, on a
+bounded sample of the same workload per step.  It is a deliberately slow program: a reported baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "candidate configs scored/s (16 dots, default algorithm, open 4x4 grid, 100x100 pixels)"
+UNIT = "candidates/s"
+FP64_OPS_PER_CANDIDATE = 3.0   # 2 DADD + 1 DSETP per candidate in the static Gray walk
+FP64_LANES_PER_SM = 64         # 148 SMs x 64 FP64 lanes x SM clock
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config4", choices=["config4", "config5"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.idx = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.idx), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workloads(name, rank):
+    from paper_2404_04994_b200 import workloads as wl
+    if name == "config4":
+        return [wl.config4(100, 100, seed=3 + 100 * rank)]          # rank r > 0: an independently seeded diagram
+    return [wl.config5_array(j + 256 * rank) for j in range(8)]     # a slice of the dataset batch (secondary bench)
+
+
+def candidates_of(wls, alg="default"):
+    return sum(w.P * (2 ** w.n_dot) for w in wls)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def run_reference(args, rank):
+    """The oracle as the reference arm (this tier has no reference implementation): rank 0 only."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_2404_04994_b200 import workloads as wl
+    w = wl.config4(100, 100)
+    m = oracle.Model(w.C_dd, w.C_gd)
+    t0 = time.perf_counter()
+    m.ground_state(w.Vg[:8])
+    per_px = (time.perf_counter() - t0) / 8
+    total_budget = 150.0
+    px = int(max(4, min(400, total_budget / max(1, args.steps + args.warmup) / per_px)))
+    rng = np.random.default_rng(0)
+    sel = np.sort(rng.choice(w.P, size=px, replace=False))
+    for _ in range(args.warmup):
+        m.ground_state(w.Vg[sel])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        m.ground_state(w.Vg[sel])
+    dt = (time.perf_counter() - t0) / args.steps
+    val = px * 65536 / dt
+    sample = f"{px} of 10000 pixels (seeded random subset) of config4 per step, single thread"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[3]: open 4x4 grid, 16 dots, default, 100x100 (sampled)",
+                       "sample": sample},
+            "pixels_per_s": px / dt,
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(args):
+    import oracle
+    from paper_2404_04994_b200 import workloads as wl
+    w = wl.config4(100, 100)
+    m = oracle.Model(w.C_dd, w.C_gd)
+    t0 = time.perf_counter()
+    m.ground_state(w.Vg[:8])
+    per_px = (time.perf_counter() - t0) / 8
+    px = int(max(8, min(1000, args.cpu_seconds / per_px)))
+    rng = np.random.default_rng(0)
+    sel = np.sort(rng.choice(w.P, size=px, replace=False))
+    t0 = time.perf_counter()
+    m.ground_state(w.Vg[sel])
+    dt = time.perf_counter() - t0
+    out = {"value": px * 65536 / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"{px} of 10000 pixels (seeded random subset) of config4, {dt:.1f} s",
+           "pixels_per_s": px / dt, "host_cores": os.cpu_count()}
+    if oracle.has_openmp() and (os.cpu_count() or 1) > 1:
+        nt = os.cpu_count()
+        px2 = int(min(4000, px * max(1, nt // 2)))
+        sel2 = np.sort(rng.choice(w.P, size=px2, replace=False))
+        t0 = time.perf_counter()
+        m.ground_state(w.Vg[sel2], n_threads=nt)
+        dt2 = time.perf_counter() - t0
+        out["all_cores"] = {"value": px2 * 65536 / dt2, "unit": UNIT, "cores": nt,
+                            "sample": f"{px2} pixels, OpenMP over pixels, {dt2:.1f} s"}
+    return out
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2404_04994_b200 import api
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    wls = make_workloads(args.workload, rank)
+    models = [api.Model(w.C_dd, w.C_gd) for w in wls]
+    Vgs = [torch.from_numpy(w.Vg).to(dev) for w in wls]
+    outs = [{"N": torch.empty((w.P, w.n_dot), dtype=torch.int32, device=dev),
+             "E": torch.empty(w.P, dtype=torch.float64, device=dev)} for w in wls]
+    cand_step = candidates_of(wls)
+    px_step = sum(w.P for w in wls)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def step():
+        for m, v, o in zip(models, Vgs, outs):
+            m.ground_state(v, out=o)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        flush.fill_(1)
+        step()
+    launches_per_step = api.last_launch_plan()[1] * len(models)
+    plan = api.last_launch_plan()[0]
+
+    # ---- timed region: K steps, CUDA events around each step on the launching stream, L2 flushed between steps ----
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)
+        ev[k][0].record()
+        step()
+        ev[k][1].record()
+    barrier()
+    clocks = sampler.stop()
+    times = np.array([a.elapsed_time(b) for a, b in ev])            # ms
+    tot_ms = float(times.sum())
+    if world > 1:
+        t = torch.tensor([tot_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tot_ms = float(t.item())
+    ms_per_step = tot_ms / args.steps
+    value = world * cand_step / (ms_per_step * 1e-3)
+
+    if rank != 0:
+        return
+
+    # ---- per-kernel share of the step: CUDA events between the kernels (separate pass, same launch configuration) --
+    kt = api.kernel_times(models[0], Vgs[0], steps=args.steps, flush=flush)
+    walk_ms = kt.get("qa_walk_kernel", 0.0)
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
+    peak_nominal = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6           # FP64 thread-inst/s
+    peak_measured = api.measure_fp64_rate(1.0)
+    alg_ops = FP64_OPS_PER_CANDIDATE * wls[0].P * (2 ** wls[0].n_dot)
+    achieved = alg_ops / (walk_ms * 1e-3) if walk_ms > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "qa_walk_kernel", "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
+                "unit": "FP64 Ginst/s", "frac": achieved / peak_nominal, "traffic": None,
+                "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max_mhz:.0f} MHz "
+                               "(DESIGN.md); MEASURED_PEAKS.json has no FP64 figure",
+                "peak_measured_dfma_probe": peak_measured / 1e9, "frac_of_measured_probe": achieved / peak_measured,
+                "fp64_ops_per_candidate": FP64_OPS_PER_CANDIDATE, "kernel_ms": walk_ms,
+                "kernel_share_of_step": walk_ms / max(1e-9, sum(kt.values())), "kernel_times_ms": kt,
+                "gflops_equiv_dadd": achieved / 1e9}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D + search + D2H inside the timed region --------
+    e2e = None
+    if not args.no_e2e:
+        hv = [torch.from_numpy(w.Vg).pin_memory() for w in wls]
+        ho = [{"N": torch.empty((w.P, w.n_dot), dtype=torch.int32).pin_memory(),
+               "E": torch.empty(w.P, dtype=torch.float64).pin_memory()} for w in wls]
+        for _ in range(3):
+            for m, v, o in zip(models, hv, ho):
+                m.ground_state_host(v, out=o)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            for m, v, o in zip(models, hv, ho):
+                m.ground_state_host(v, out=o)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / args.steps
+        e2e = {"value": cand_step / dt, "unit": UNIT, "ms_per_step": dt * 1e3,
+               "h2d_bytes_per_step": int(sum(v.numel() * 8 for v in hv)),
+               "d2h_bytes_per_step": int(sum(o["N"].numel() * 4 + o["E"].numel() * 8 for o in ho)),
+               "api": "qa_ground_state_host (pinned host buffers)", "n_gpus_measured": 1}
+
+    cpu = None if args.no_cpu_baseline else cpu_baseline(args)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[3]: open 4x4 grid, 16 dots, default algorithm, 100x100 pixels, "
+                                   "2^16 candidates/pixel, seed 3" if args.workload == "config4" else
+                                   "BASELINE.json configs[4] slice: 8 open 8-dot arrays, 128x128, default",
+                       "pixels_per_step_per_gpu": px_step, "candidates_per_step_per_gpu": cand_step,
+                       "l2": "flushed (256 MiB write) between timed steps", "parallelism": f"pixel-range x{world}"},
+            "pixels_per_s": world * px_step / (ms_per_step * 1e-3), "diagram_ms": ms_per_step,
+            "ms_per_step_min": float(times.min()), "ms_per_step_median": float(np.median(times)),
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+            "kernels_per_step": plan, "clocks": clocks,
+            "paper_context": "paper: same diagram shape in < 1 s on a GTX 1080 Ti via JAX (PAPER.md L7, L498)"}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    import __graft_entry__ as ge
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl")
+        dist.barrier()
+    run_ours(args, rank, world, local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

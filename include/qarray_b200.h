@@ -137,6 +137,13 @@ QA_API qa_status qa_ground_state_host(const qa_model *model, const double *h_Vg,
  * Returns FP64 thread-instructions per second (1 DFMA = 1) -- the denominator of the ALU roofline. */
 QA_API qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *cuda_stream);
 
+/* Per-kernel timing of a call (measurement aid, per host thread).  While enabled, qa_ground_state_open / _closed record
+ * CUDA events on the call's stream before the first and after every kernel.  qa_get_kernel_timings waits for the last
+ * event of the most recent call and returns the device time of each of its kernels in milliseconds, in launch order
+ * (names: qa_last_launch_plan).  ms: host, max_kernels floats; *n_kernels: how many were written. */
+QA_API qa_status qa_set_kernel_timing(int enable);
+QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernels);
+
 /* Names of the kernels the last ground-state call on this host thread enqueued (comma separated; static storage). */
 QA_API const char *qa_last_launch_plan(void);
 /* Number of kernels the last ground-state call on this host thread enqueued. */

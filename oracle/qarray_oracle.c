@@ -212,6 +212,7 @@ static int eqp_solve(const qo_model *m, const double *c, const int *W, int close
         }
         *lambda = (Nhat - su) / sw;
         for (int a = 0; a < k; a++) u[a] += *lambda * w[a];
+        if (k == 1) u[0] = Nhat; /* reading R3: a single free dot carries the whole charge, exactly (1^T x = N_hat) */
     }
     for (int a = 0; a < k; a++) xh[F[a]] = u[a];
     return 0;

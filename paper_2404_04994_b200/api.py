@@ -22,7 +22,8 @@ STATUS_NAMES = ["QA_OK", "QA_ERR_INVALID_ARG", "QA_ERR_NOT_SYMMETRIC", "QA_ERR_N
                 "QA_ERR_INFEASIBLE", "QA_ERR_OVERFLOW", "QA_ERR_CUDA", "QA_ERR_UNSUPPORTED"]
 EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "qa_model_n_dot", "qa_model_n_gate",
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
-           "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_last_launch_plan",
+           "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
+           "qa_get_kernel_timings", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
 
 
@@ -71,6 +72,8 @@ def lib() -> C.CDLL:
         l.qa_ground_state_host.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, vp, vp, vp,
                                            vp, vp]
         l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
+        l.qa_set_kernel_timing.argtypes = [C.c_int]
+        l.qa_get_kernel_timings.argtypes = [C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_int)]
         l.qa_last_launch_plan.restype = C.c_char_p
         l.qa_status_string.restype = C.c_char_p
         l.qa_status_string.argtypes = [C.c_int]
@@ -224,6 +227,28 @@ def measure_fp64_rate(seconds: float = 1.0) -> float:
     _check(lib().qa_measure_fp64_rate(float(seconds), C.byref(r), C.c_void_p(torch.cuda.current_stream().cuda_stream)),
            "qa_measure_fp64_rate")
     return r.value
+
+
+def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch.Tensor | None = None, **kw) -> dict:
+    """Average device time (ms) of each kernel of model.ground_state(Vg, **kw), from CUDA events recorded by the library
+    between its kernels on the launching stream (qa_set_kernel_timing / qa_get_kernel_timings)."""
+    acc: dict = {}
+    lib().qa_set_kernel_timing(1)
+    try:
+        for k in range(steps):
+            if flush is not None:
+                flush.fill_(k & 0xff)
+            model.ground_state(Vg, **kw)
+            ms = (C.c_float * 8)()
+            n = C.c_int()
+            _check(lib().qa_get_kernel_timings(8, ms, C.byref(n)), "qa_get_kernel_timings")
+            names = last_launch_plan()[0]
+            for i in range(n.value):
+                key = names[i].split("<")[0]
+                acc[key] = acc.get(key, 0.0) + ms[i] / steps
+    finally:
+        lib().qa_set_kernel_timing(0)
+    return acc
 
 
 def last_launch_plan():

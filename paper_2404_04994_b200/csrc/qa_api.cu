@@ -28,6 +28,19 @@ namespace {
 thread_local std::string g_plan;
 thread_local int g_plan_count = 0;
 thread_local char g_cuda_err[256] = "";
+thread_local bool g_timing = false;           // measurement aid: CUDA events around every kernel of a call
+thread_local cudaEvent_t g_events[8];
+thread_local int g_n_events_created = 0, g_n_marks = 0;
+
+void timing_mark(cudaStream_t stream)
+{
+    if (!g_timing || g_n_marks >= 8) return;
+    if (g_n_marks >= g_n_events_created) {
+        if (cudaEventCreate(&g_events[g_n_events_created]) != cudaSuccess) return;
+        ++g_n_events_created;
+    }
+    cudaEventRecord(g_events[g_n_marks++], stream);
+}
 
 qa_status cuda_fail(cudaError_t e, const char *where)
 {
@@ -180,7 +193,10 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     carve(m, P, d_ws, &ws);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
     QaCallArgs a{closed, N_hat, (int)alg, t, n_max};
+    g_n_marks = 0;
+    timing_mark(stream);
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
+    timing_mark(stream);
     if (alg == QA_ALG_DEFAULT && !closed) {
         QA_CUDA(qa_launch_walk(m->dev, n, m->walk, ws, d_stats, m->sm_count, stream));
     } else {
@@ -189,7 +205,9 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
                                                   : std::pow(1.0 + t, (double)n);
         QA_CUDA(qa_launch_enumerate(m->dev, n, ws, a, expect, d_stats, stream));
     }
+    timing_mark(stream);
     QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream));
+    timing_mark(stream);
     return QA_OK;
 }
 
@@ -411,6 +429,26 @@ qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *
     cudaFree(sink);
     *thread_inst_per_s = rate;
     return st;
+}
+
+qa_status qa_set_kernel_timing(int enable)
+{
+    g_timing = enable != 0;
+    g_n_marks = 0;
+    return QA_OK;
+}
+
+qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernels)
+{
+    if (!ms || !n_kernels || max_kernels < 0) return QA_ERR_INVALID_ARG;
+    *n_kernels = 0;
+    if (g_n_marks < 2) return QA_OK;
+    QA_CUDA(cudaEventSynchronize(g_events[g_n_marks - 1]));
+    for (int k = 0; k + 1 < g_n_marks && k < max_kernels; ++k) {
+        QA_CUDA(cudaEventElapsedTime(&ms[k], g_events[k], g_events[k + 1]));
+        *n_kernels = k + 1;
+    }
+    return QA_OK;
 }
 
 const char *qa_last_launch_plan(void) { return g_plan.c_str(); }

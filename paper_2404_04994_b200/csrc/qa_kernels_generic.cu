@@ -116,6 +116,7 @@ __device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool 
                 for (int f2 = 0; f2 < N; ++f2)
                     if (!((A >> f2) & 1u)) rowF += sC[f * N + f2];
                 s += lam * rowF;
+                if (k == N - 1) s = Nhat;  // R3: a single free dot carries the whole charge, exactly
             }
             x[f] = s;
         }
