@@ -23,7 +23,7 @@ STATUS_NAMES = ["QA_OK", "QA_ERR_INVALID_ARG", "QA_ERR_NOT_SYMMETRIC", "QA_ERR_N
 EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "qa_model_n_dot", "qa_model_n_gate",
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
            "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
-           "qa_get_kernel_timings", "qa_last_launch_plan",
+           "qa_get_kernel_timings", "qa_set_walk_variant", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
 
 
@@ -73,6 +73,7 @@ def lib() -> C.CDLL:
                                            vp, vp]
         l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
         l.qa_set_kernel_timing.argtypes = [C.c_int]
+        l.qa_set_walk_variant.argtypes = [C.c_int]
         l.qa_get_kernel_timings.argtypes = [C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_int)]
         l.qa_last_launch_plan.restype = C.c_char_p
         l.qa_status_string.restype = C.c_char_p
@@ -249,6 +250,11 @@ def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch
     finally:
         lib().qa_set_kernel_timing(0)
     return acc
+
+
+def set_walk_variant(variant: int) -> None:
+    """qa_set_walk_variant: choose the kernel that scores open/default candidates for n_dot >= 13 (measurement aid)."""
+    _check(lib().qa_set_walk_variant(int(variant)), "qa_set_walk_variant")
 
 
 def last_launch_plan():

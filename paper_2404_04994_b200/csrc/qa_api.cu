@@ -2,6 +2,7 @@
 // workspace carving and kernel dispatch.  No compute on the host beyond S0; no CPU fallback.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -139,6 +140,20 @@ qa_status rebuild(qa_model *m)
     return QA_OK;
 }
 
+// qa_set_walk_variant (measurement aid): which kernel scores the open/default candidates of arrays with n >= 13.
+// 0 = exact-compare walk (the n <= 12 kernel), 1 = filtered walk + finish kernel + separate finalize, 2 (default) =
+// filtered walk + finish kernel with fused S7, 3 = as 2 with the walk compiled for 4 instead of 3 CTAs/SM.  Initial value from the environment variable QA_WALK_VARIANT.
+int g_walk_variant = -1;
+int walk_variant()
+{
+    if (g_walk_variant < 0) {
+        const char *e = std::getenv("QA_WALK_VARIANT");
+        g_walk_variant = e ? std::atoi(e) : 2;
+        if (g_walk_variant < 0 || g_walk_variant > 3) g_walk_variant = 2;
+    }
+    return g_walk_variant;
+}
+
 size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
@@ -157,6 +172,9 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
     int32_t *ct = static_cast<int32_t *>(take(n * Pz * 4));
     uint64_t *tt = static_cast<uint64_t *>(take(Pz * 8));
     uint64_t *be = static_cast<uint64_t *>(take(Pz * 8));
+    double *e0 = static_cast<double *>(take(Pz * 8));
+    uint2 *rec = static_cast<uint2 *>(take(n >= 13 ? Pz * 8 * ((size_t)1 << (n - 13)) : 0));
+    double *sv = static_cast<double *>(take(n >= 13 ? Pz * 72 * ((size_t)1 << (n - 13)) : 0));
     if (ws) {
         ws->h = h;
         ws->nc = nc;
@@ -164,6 +182,9 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
         ws->cnt = ct;
         ws->total = tt;
         ws->best = be;
+        ws->e0 = e0;
+        ws->rec = rec;
+        ws->sv = sv;
         ws->P = P;
     }
     return off;
@@ -197,15 +218,22 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     timing_mark(stream);
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
     timing_mark(stream);
-    if (alg == QA_ALG_DEFAULT && !closed) {
+    if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && walk_variant() != 0) {
+        const bool fuse = m->ns == 0 && walk_variant() != 1;  // S7 runs inside the finish kernel: no finalize launch
+        QA_CUDA(qa_launch_filter_walk(m->dev, n, m->walk, ws, d_Vg, fuse ? d_N : nullptr, d_E, nullptr, m->sm_count,
+                                      walk_variant(), stream));
+        timing_mark(stream);
+        if (fuse) return QA_OK;
+    } else if (alg == QA_ALG_DEFAULT && !closed) {
         QA_CUDA(qa_launch_walk(m->dev, n, m->walk, ws, d_stats, m->sm_count, stream));
+        timing_mark(stream);
     } else {
         double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n)
                         : alg == QA_ALG_DEFAULT   ? std::pow(2.0, (double)n)
                                                   : std::pow(1.0 + t, (double)n);
         QA_CUDA(qa_launch_enumerate(m->dev, n, ws, a, expect, d_stats, stream));
+        timing_mark(stream);
     }
-    timing_mark(stream);
     QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream));
     timing_mark(stream);
     return QA_OK;
@@ -213,6 +241,7 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
 
 }  // namespace
 
+void qa_timing_mark(cudaStream_t stream) { timing_mark(stream); }
 void qa_plan_reset()
 {
     g_plan.clear();
@@ -435,6 +464,13 @@ qa_status qa_set_kernel_timing(int enable)
 {
     g_timing = enable != 0;
     g_n_marks = 0;
+    return QA_OK;
+}
+
+qa_status qa_set_walk_variant(int variant)
+{
+    if (variant < 0 || variant > 3) return QA_ERR_INVALID_ARG;
+    g_walk_variant = variant;
     return QA_OK;
 }
 

@@ -38,6 +38,9 @@ struct QaWorkspace {
     int32_t *cnt;     // [n][P]  number of candidate values of dot i (1, 2, n_max + 1, or up to 4 when widened)
     uint64_t *total;  // [P]     product of cnt = size of the enumerated set
     uint64_t *best;   // [P]     mixed-radix index (dot 0 most significant) of the argmin, ~0 if the set is empty
+    double *e0;       // [P]     E(base) = 1/2 (base - N_c)^T M (base - N_c) >= 0, the energy of the base point
+    uint2 *rec;       // [P][2^(n-13)]  filtered walk: per warp of the pixel (min of hi32(e), ballot of the lanes attaining it)
+    double *sv;       // [P][2^(n-13)][9]  filtered walk: h'[0..7] and start value of the first such lane of each warp
     int64_t P;
 };
 
@@ -58,6 +61,7 @@ struct QaWalkTable {
 // launch-plan log (host, thread-local; filled by the launchers)
 void qa_plan_reset();
 void qa_plan_add(const char *kernel_name);
+void qa_timing_mark(cudaStream_t stream);  // measurement aid: event between two kernels of a call (no-op unless enabled)
 
 // launchers (each enqueues exactly one kernel on `stream` and logs it)
 cudaError_t qa_launch_prologue(const QaDevModel *d_model, int n, int g, const double *d_Vg, QaWorkspace ws,
@@ -66,6 +70,9 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
                                 qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, qa_stats *d_stats,
                            int sm_count, cudaStream_t stream);
+cudaError_t qa_launch_filter_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws,
+                                  const double *d_Vg, int32_t *d_N, double *d_E, double *d_Vs, int sm_count, int variant,
+                                  cudaStream_t stream);
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
                                double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int iters, cudaStream_t stream);
@@ -91,6 +98,81 @@ __device__ __forceinline__ void qa_lexmin(double &e, uint64_t &i, double e2, uin
     if (e2 < e || (e2 == e && i2 < i)) {
         e = e2;
         i = i2;
+    }
+}
+// S7 + S8 for one pixel, one thread: N* = base + digits of the winning mixed-radix index `idx`; E(N*) recomputed from the
+// definition (Eq. (C1)); sensor dots (L149 + Eq. (3), reading R8).  idx = ~0: empty candidate set.
+__device__ __forceinline__ void qa_finalize_pixel(const QaDevModel *__restrict__ mdl, const double *__restrict__ Vg,
+                                                  const QaWorkspace &ws, int64_t p, uint64_t idx,
+                                                  int32_t *__restrict__ outN, double *__restrict__ outE,
+                                                  double *__restrict__ outVs)
+{
+    const int64_t P = ws.P;
+    const int n = mdl->n, nf = mdl->nf, ns = mdl->ns, g = mdl->g;
+    int32_t Ns[QA_MAXN];
+    double d[QA_MAXN];
+    const bool empty = idx == ~0ull;
+    for (int i = n - 1; i >= 0; --i) {
+        const uint64_t c = (uint64_t)ws.cnt[i * P + p];
+        const int32_t dgt = (int32_t)(idx % c);
+        idx /= c;
+        Ns[i] = empty ? -1 : ws.base[i * P + p] + dgt;
+        d[i] = (double)Ns[i] - ws.nc[i * P + p];
+    }
+    double E = 0.0;
+    for (int i = 0; i < n; ++i) {
+        double row = 0.0;
+        for (int j = 0; j < n; ++j) row = fma(mdl->M[i * QA_MAXN + j], d[j], row);
+        E = fma(d[i], row, E);
+    }
+    outE[p] = empty ? INFINITY : 0.5 * E;
+    if (ns == 0) {
+        for (int i = 0; i < n; ++i) outN[p * n + i] = Ns[i];
+        return;
+    }
+    // full model: N_c of every dot (same fma order), array dots fixed, then each sensor independently
+    double ncf[QA_MAXN], df[QA_MAXN];
+    int32_t Nf[QA_MAXN];
+    for (int i = 0; i < nf; ++i) {
+        double acc = 0.0;
+        for (int k = 0; k < g; ++k) acc = fma(mdl->Cgdf[i * QA_MAXG + k], __ldg(Vg + p * g + k), acc);
+        ncf[i] = acc;
+        df[i] = 0.0;
+        Nf[i] = 0;
+    }
+    for (int a = 0; a < n; ++a) {
+        const int i = mdl->arr_idx[a];
+        Nf[i] = Ns[a];
+        df[i] = (double)Ns[a] - ncf[i];
+    }
+    for (int a = 0; a < ns; ++a) {
+        const int s = mdl->sens_idx[a];
+        double y = 0.0;
+        for (int b = 0; b < n; ++b) {
+            const int j = mdl->arr_idx[b];
+            y += mdl->Mf[s * QA_MAXN + j] * df[j];
+        }
+        const double Mss = mdl->Mf[s * QA_MAXN + s];
+        const double sstar = ncf[s] - y / Mss;
+        const double fl = floor(sstar);
+        const int32_t c0 = fl > 0.0 ? (int32_t)fl : 0;
+        const double d0 = (double)c0 - ncf[s], d1 = (double)(c0 + 1) - ncf[s];
+        const double e0 = d0 * y + 0.5 * Mss * d0 * d0;
+        const double e1 = d1 * y + 0.5 * Mss * d1 * d1;
+        Nf[s] = e1 < e0 ? c0 + 1 : c0;
+    }
+    for (int a = 0; a < ns; ++a) {
+        const int s = mdl->sens_idx[a];
+        df[s] = (double)Nf[s] - ncf[s];
+    }
+    for (int i = 0; i < nf; ++i) outN[p * nf + i] = Nf[i];
+    if (outVs) {
+        for (int a = 0; a < ns; ++a) {
+            const int s = mdl->sens_idx[a];
+            double vsum = 0.0;
+            for (int j = 0; j < nf; ++j) vsum += mdl->Mf[s * QA_MAXN + j] * df[j];
+            outVs[p * ns + a] = vsum;
+        }
     }
 }
 #endif

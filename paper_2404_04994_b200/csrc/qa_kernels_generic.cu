@@ -245,17 +245,20 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
         total *= (uint64_t)cnt[i];
     }
     if (live) {
+        double e0 = 0.0;
 #pragma unroll
         for (int i = 0; i < N; ++i) {
             double gi = 0.0;
 #pragma unroll
             for (int j = 0; j < N; ++j) gi = fma(sM[i * N + j], d0[j], gi);
+            e0 = fma(d0[i], gi, e0);
             ws.h[i * P + p] = gi + 0.5 * sM[i * N + i];
             ws.nc[i * P + p] = nc[i];
             ws.base[i * P + p] = base[i];
             ws.cnt[i * P + p] = cnt[i];
         }
         ws.total[p] = total;
+        ws.e0[p] = 0.5 * e0;
         if (xcont) {
 #pragma unroll
             for (int i = 0; i < N; ++i) xcont[p * N + i] = x[i];
@@ -396,83 +399,15 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Finalize: one thread per pixel.  S7: N* = base + digits of the winning index; E(N*) recomputed from the definition
-// (Eq. (C1)).  S8 (sensor dots, L149 + Eq. (3), reading R8).
+// Finalize: one thread per pixel (qa_finalize_pixel in qa_internal.cuh).
 __global__ void __launch_bounds__(FIN_THREADS) qa_finalize_kernel(const QaDevModel *__restrict__ mdl,
                                                                   const double *__restrict__ Vg, QaWorkspace ws,
                                                                   int32_t *__restrict__ outN, double *__restrict__ outE,
                                                                   double *__restrict__ outVs)
 {
-    const int64_t P = ws.P;
     const int64_t p = blockIdx.x * (int64_t)FIN_THREADS + threadIdx.x;
-    if (p >= P) return;
-    const int n = mdl->n, nf = mdl->nf, ns = mdl->ns, g = mdl->g;
-    int32_t Ns[QA_MAXN];
-    double d[QA_MAXN];
-    uint64_t idx = ws.best[p];
-    const bool empty = idx == ~0ull;
-    for (int i = n - 1; i >= 0; --i) {
-        const uint64_t c = (uint64_t)ws.cnt[i * P + p];
-        const int32_t dgt = (int32_t)(idx % c);
-        idx /= c;
-        Ns[i] = empty ? -1 : ws.base[i * P + p] + dgt;
-        d[i] = (double)Ns[i] - ws.nc[i * P + p];
-    }
-    double E = 0.0;
-    for (int i = 0; i < n; ++i) {
-        double row = 0.0;
-        for (int j = 0; j < n; ++j) row = fma(mdl->M[i * QA_MAXN + j], d[j], row);
-        E = fma(d[i], row, E);
-    }
-    outE[p] = empty ? INFINITY : 0.5 * E;
-    if (ns == 0) {
-        for (int i = 0; i < n; ++i) outN[p * n + i] = Ns[i];
-        return;
-    }
-    // full model: N_c of every dot (same fma order), array dots fixed, then each sensor independently
-    double ncf[QA_MAXN], df[QA_MAXN];
-    int32_t Nf[QA_MAXN];
-    for (int i = 0; i < nf; ++i) {
-        double acc = 0.0;
-        for (int k = 0; k < g; ++k) acc = fma(mdl->Cgdf[i * QA_MAXG + k], __ldg(Vg + p * g + k), acc);
-        ncf[i] = acc;
-        df[i] = 0.0;
-        Nf[i] = 0;
-    }
-    for (int a = 0; a < n; ++a) {
-        const int i = mdl->arr_idx[a];
-        Nf[i] = Ns[a];
-        df[i] = (double)Ns[a] - ncf[i];
-    }
-    for (int a = 0; a < ns; ++a) {
-        const int s = mdl->sens_idx[a];
-        double y = 0.0;
-        for (int b = 0; b < n; ++b) {
-            const int j = mdl->arr_idx[b];
-            y += mdl->Mf[s * QA_MAXN + j] * df[j];
-        }
-        const double Mss = mdl->Mf[s * QA_MAXN + s];
-        const double sstar = ncf[s] - y / Mss;
-        const double fl = floor(sstar);
-        const int32_t c0 = fl > 0.0 ? (int32_t)fl : 0;
-        const double d0 = (double)c0 - ncf[s], d1 = (double)(c0 + 1) - ncf[s];
-        const double e0 = d0 * y + 0.5 * Mss * d0 * d0;
-        const double e1 = d1 * y + 0.5 * Mss * d1 * d1;
-        Nf[s] = e1 < e0 ? c0 + 1 : c0;
-    }
-    for (int a = 0; a < ns; ++a) {
-        const int s = mdl->sens_idx[a];
-        df[s] = (double)Nf[s] - ncf[s];
-    }
-    for (int i = 0; i < nf; ++i) outN[p * nf + i] = Nf[i];
-    if (outVs) {
-        for (int a = 0; a < ns; ++a) {
-            const int s = mdl->sens_idx[a];
-            double vsum = 0.0;
-            for (int j = 0; j < nf; ++j) vsum += mdl->Mf[s * QA_MAXN + j] * df[j];
-            outVs[p * ns + a] = vsum;
-        }
-    }
+    if (p >= ws.P) return;
+    qa_finalize_pixel(mdl, Vg, ws, p, ws.best[p], outN, outE, outVs);
 }
 
 // FP64 issue-rate probe: 8 independent DFMA chains per thread.

@@ -97,8 +97,30 @@ def test_config4_open_grid16_default(api, W, H):
     """n = 16, 2^16 candidates per pixel: the hot kernel (NL = 8, NH = 8), QP pixels included."""
     w = wl.config4(W, H)
     rep, g, o = check(api, w, algorithm="default")
-    assert g["plan"][0] == ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"]
+    assert g["plan"][0] == ["qa_prologue_kernel", "qa_filter_walk_kernel", "qa_filter_finish_kernel"]
     assert g["stats"]["n_candidates_scored"] == w.P * 65536
+
+
+@pytest.mark.parametrize("n", [13, 14, 16])
+def test_walk_variants_agree(api, n):
+    """The exact-compare walk, the filtered walk with a separate finalize and the fused filtered walk give the same
+    charge map and the same energies up to the summation order of E(N*); each is also checked against the oracle."""
+    w = wl.random_open(n, n, 45, seed=200 + n)
+    ref = None
+    try:
+        for variant in (0, 1, 2, 3):
+            api.set_walk_variant(variant)
+            rep, g, o = check(api, w, algorithm="default")
+            names = g["plan"][0]
+            assert names[1] == ("qa_walk_kernel" if variant == 0 else "qa_filter_walk_kernel")
+            assert len(names) == {0: 3, 1: 4, 2: 3, 3: 3}[variant]
+            if ref is None:
+                ref = g
+            else:
+                assert np.array_equal(ref["N"], g["N"])
+                assert np.allclose(ref["E"], g["E"], rtol=1e-13, atol=1e-13 * g["EC"])
+    finally:
+        api.set_walk_variant(2)
 
 
 def test_config5_open_grid8_default_and_thresholded(api):
@@ -110,9 +132,9 @@ def test_config5_open_grid8_default_and_thresholded(api):
 
 
 # ---- every n_dot through the static walk and the generic enumeration ----------------------------------------------
-@pytest.mark.parametrize("n", list(range(1, 13)))
+@pytest.mark.parametrize("n", list(range(1, 17)))
 def test_all_sizes_default_open(api, n):
-    w = wl.random_open(n, n + (n % 3), 301 if n <= 10 else 67, seed=50 + n)
+    w = wl.random_open(n, n + (n % 3), 301 if n <= 10 else (67 if n <= 13 else 37), seed=50 + n)
     check(api, w, algorithm="default")
 
 
