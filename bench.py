@@ -28,7 +28,7 @@ import numpy as np  # noqa: E402
 
 METRIC = "candidate configs scored/s (16 dots, default algorithm, open 4x4 grid, 100x100 pixels)"
 UNIT = "candidates/s"
-FP64_OPS_PER_CANDIDATE = 2.0   # 2 DADD per candidate in the filtered Gray walk (min is integer)
+FP64_OPS_PER_CANDIDATE = 334.0 / 256.0   # FP64-pipe instructions per candidate of the min-plus walk
 FP64_LANES_PER_SM = 64         # 148 SMs x 64 FP64 lanes x SM clock
 
 
@@ -220,8 +220,8 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- per-kernel share of the step: CUDA events between the kernels (separate pass, same launch configuration) --
     kt = api.kernel_times(models[0], Vgs[0], steps=args.steps, flush=flush)
-    hot = "qa_filter_walk_kernel" if "qa_filter_walk_kernel" in kt else "qa_walk_kernel"
-    ops_per_cand = FP64_OPS_PER_CANDIDATE if hot == "qa_filter_walk_kernel" else 3.0
+    hot = "qa_minplus_walk_kernel" if "qa_minplus_walk_kernel" in kt else "qa_walk_kernel"
+    ops_per_cand = FP64_OPS_PER_CANDIDATE if hot == "qa_minplus_walk_kernel" else 3.0
     walk_ms = kt.get(hot, 0.0)                                     # pass 1 only; the finish kernel is listed beside it
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0

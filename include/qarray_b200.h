@@ -144,10 +144,9 @@ QA_API qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s,
 QA_API qa_status qa_set_kernel_timing(int enable);
 QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernels);
 
-/* Which kernel scores the 2^n candidates of the open default algorithm for n_dot >= 13 (process-wide; measurement and
- * cross-check aid, results are identical): 0 = the exact-compare Gray walk used for n_dot <= 12, 1 = filtered walk and
- * finish kernel followed by the generic finalize kernel, 2 = filtered walk and finish kernel with fused outputs (default),
- * 3 = as 2 with the walk compiled for a higher occupancy target.  Returns QA_ERR_INVALID_ARG outside 0..3. */
+/* Which kernel scores the 2^n candidates of the open default algorithm for n_dot >= 13 (process-wide; cross-check aid,
+ * the results are identical): 0 = the exact-compare Gray walk used for n_dot <= 12, 1 (default) = the min-plus walk with
+ * its finish kernel.  Returns QA_ERR_INVALID_ARG for any other value. */
 QA_API qa_status qa_set_walk_variant(int variant);
 
 /* Names of the kernels the last ground-state call on this host thread enqueued (comma separated; static storage). */

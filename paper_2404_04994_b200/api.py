@@ -253,7 +253,7 @@ def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch
 
 
 def set_walk_variant(variant: int) -> None:
-    """qa_set_walk_variant: choose the kernel that scores open/default candidates for n_dot >= 13 (measurement aid)."""
+    """qa_set_walk_variant: 0 = exact-compare Gray walk, 1 = min-plus walk (default) for n_dot >= 13 (cross-check aid)."""
     _check(lib().qa_set_walk_variant(int(variant)), "qa_set_walk_variant")
 
 

@@ -127,29 +127,47 @@ qa_status rebuild(qa_model *m)
         for (int k = 0; k < g; ++k) h.Cgdf[i * QA_MAXG + k] = m->Cgdf[i * g + k];
     }
     // pair table of the low bits: low bit j <-> search dot n-1-j
-    const int nl = n < QA_WALK_NL ? n : QA_WALK_NL;
-    for (int b = 0; b < (1 << QA_WALK_NL); ++b) {
+    const int nl = n < QA_PAIR_NL ? n : QA_PAIR_NL;
+    for (int b = 0; b < (1 << QA_PAIR_NL); ++b) {
         double s = 0.0;
         if (b < (1 << nl))
             for (int j = 0; j < nl; ++j)
                 for (int j2 = j + 1; j2 < nl; ++j2)
                     if (((b >> j) & 1) && ((b >> j2) & 1)) s += Msub[(n - 1 - j) * n + (n - 1 - j2)];
-        m->walk.QL[b] = s;
+        h.QL[b] = s;
+        if (b < (1 << QA_WALK_NL)) m->walk.QL[b] = s;
+    }
+    // tables of the min-plus walk: high pattern t of the NH = n - QA_WALK_NL high bits (high bit jh <-> dot n-1-NL-jh)
+    if (n > QA_WALK_NL) {
+        const int NL = QA_WALK_NL, NH = n - NL;
+        for (int t = 0; t < (1 << NH); ++t) {
+            for (int j = 0; j < NL; ++j) {
+                double s = 0.0;
+                for (int jh = 0; jh < NH; ++jh)
+                    if ((t >> jh) & 1) s += Msub[(n - 1 - j) * n + (n - 1 - NL - jh)];
+                h.VT[t * NL + j] = s;
+            }
+            double q = h.EC;
+            for (int jh = 0; jh < NH; ++jh)
+                for (int jh2 = jh + 1; jh2 < NH; ++jh2)
+                    if (((t >> jh) & 1) && ((t >> jh2) & 1)) q += Msub[(n - 1 - NL - jh) * n + (n - 1 - NL - jh2)];
+            h.QHT[t] = q;
+        }
     }
     QA_CUDA(cudaMemcpy(m->dev, &h, sizeof(h), cudaMemcpyHostToDevice));
     return QA_OK;
 }
 
-// qa_set_walk_variant (measurement aid): which kernel scores the open/default candidates of arrays with n >= 13.
-// 0 = exact-compare walk (the n <= 12 kernel), 1 = filtered walk + finish kernel + separate finalize, 2 (default) =
-// filtered walk + finish kernel with fused S7, 3 = as 2 with the walk compiled for 4 instead of 3 CTAs/SM.  Initial value from the environment variable QA_WALK_VARIANT.
+// qa_set_walk_variant (cross-check aid): which kernel scores the open/default candidates of arrays with n >= 13.
+// 0 = exact-compare Gray walk (the n <= 12 kernel), 1 (default) = min-plus walk + finish kernel.  Initial value from the
+// environment variable QA_WALK_VARIANT.
 int g_walk_variant = -1;
 int walk_variant()
 {
     if (g_walk_variant < 0) {
         const char *e = std::getenv("QA_WALK_VARIANT");
-        g_walk_variant = e ? std::atoi(e) : 2;
-        if (g_walk_variant < 0 || g_walk_variant > 3) g_walk_variant = 2;
+        g_walk_variant = e ? std::atoi(e) : 1;
+        if (g_walk_variant < 0 || g_walk_variant > 1) g_walk_variant = 1;
     }
     return g_walk_variant;
 }
@@ -174,7 +192,6 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
     uint64_t *be = static_cast<uint64_t *>(take(Pz * 8));
     double *e0 = static_cast<double *>(take(Pz * 8));
     uint2 *rec = static_cast<uint2 *>(take(n >= 13 ? Pz * 8 * ((size_t)1 << (n - 13)) : 0));
-    double *sv = static_cast<double *>(take(n >= 13 ? Pz * 72 * ((size_t)1 << (n - 13)) : 0));
     if (ws) {
         ws->h = h;
         ws->nc = nc;
@@ -184,7 +201,6 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
         ws->best = be;
         ws->e0 = e0;
         ws->rec = rec;
-        ws->sv = sv;
         ws->P = P;
     }
     return off;
@@ -219,9 +235,8 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
     timing_mark(stream);
     if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && walk_variant() != 0) {
-        const bool fuse = m->ns == 0 && walk_variant() != 1;  // S7 runs inside the finish kernel: no finalize launch
-        QA_CUDA(qa_launch_filter_walk(m->dev, n, m->walk, ws, d_Vg, fuse ? d_N : nullptr, d_E, nullptr, m->sm_count,
-                                      walk_variant(), stream));
+        const bool fuse = m->ns == 0;  // S7 runs inside the finish kernel: no finalize launch
+        QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count, stream));
         timing_mark(stream);
         if (fuse) return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && !closed) {
@@ -469,7 +484,7 @@ qa_status qa_set_kernel_timing(int enable)
 
 qa_status qa_set_walk_variant(int variant)
 {
-    if (variant < 0 || variant > 3) return QA_ERR_INVALID_ARG;
+    if (variant < 0 || variant > 1) return QA_ERR_INVALID_ARG;
     g_walk_variant = variant;
     return QA_OK;
 }

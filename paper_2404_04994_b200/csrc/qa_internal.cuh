@@ -9,6 +9,7 @@
 constexpr int QA_MAXN = 16;  // dots
 constexpr int QA_MAXG = 64;  // gates
 constexpr int QA_WALK_NL = 8;  // low bits walked per thread by the static Gray walk (2^8 candidates per thread)
+constexpr int QA_PAIR_NL = 10; // low bits covered by the model's pair-energy table QL (min-plus walk: NL <= 10)
 
 // Pixel-independent model constants in device global memory (one per qa_model).
 // "search" model = the model the candidate search runs on: the full model, or (sensor dots set) the sub-blocks of the
@@ -28,6 +29,15 @@ struct QaDevModel {
     double Cgdf[QA_MAXN * QA_MAXG]; // full c_gd
     int arr_idx[QA_MAXN];           // search dot a -> dot index in the full model
     int sens_idx[QA_MAXN];          // sensor s -> dot index in the full model
+    // QL[b] = sum_{j<j', both set in b} M[n-1-j][n-1-j']: pair energy of the low-bit pattern b (low bit j <-> search dot
+    // n-1-j), j ascending then j' ascending; entries with a bit >= n set are 0.  The table of NL < QA_PAIR_NL bits is
+    // its prefix.
+    double QL[1 << QA_PAIR_NL];
+    // Min-plus walk (n >= 13; NL = QA_WALK_NL low bits per thread, NH = n - NL high bits = one thread per pattern t):
+    //   VT[t][j] = sum over the high bits jh of t (ascending) of M[n-1-j][n-1-NL-jh]      cross term of t with low bit j
+    //   QHT[t]   = E_C + sum_{jh<jh' in t} M[n-1-NL-jh][n-1-NL-jh']                       pair energy of t, plus E_C
+    double VT[(1 << QA_WALK_NL) * QA_WALK_NL];
+    double QHT[1 << QA_WALK_NL];
 };
 
 // Per-call scratch, structure-of-arrays over pixels ([i][P] so that thread-per-pixel accesses coalesce).
@@ -39,8 +49,7 @@ struct QaWorkspace {
     uint64_t *total;  // [P]     product of cnt = size of the enumerated set
     uint64_t *best;   // [P]     mixed-radix index (dot 0 most significant) of the argmin, ~0 if the set is empty
     double *e0;       // [P]     E(base) = 1/2 (base - N_c)^T M (base - N_c) >= 0, the energy of the base point
-    uint2 *rec;       // [P][2^(n-13)]  filtered walk: per warp of the pixel (min of hi32(e), ballot of the lanes attaining it)
-    double *sv;       // [P][2^(n-13)][9]  filtered walk: h'[0..7] and start value of the first such lane of each warp
+    uint2 *rec;       // [P][2^(n-13)]  min-plus walk: per warp of the pixel (min of L over its lanes, ballot of lanes near it)
     int64_t P;
 };
 
@@ -70,9 +79,8 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
                                 qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, qa_stats *d_stats,
                            int sm_count, cudaStream_t stream);
-cudaError_t qa_launch_filter_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws,
-                                  const double *d_Vg, int32_t *d_N, double *d_E, double *d_Vs, int sm_count, int variant,
-                                  cudaStream_t stream);
+cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
+                                   double *d_E, int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
                                double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int iters, cudaStream_t stream);

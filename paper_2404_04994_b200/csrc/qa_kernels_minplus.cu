@@ -1,0 +1,457 @@
+// qa_kernels_minplus.cu -- the hot path for n >= 13: default algorithm, open array (S5 + S6 [+ S7] of SURVEY.md section
+// 8(a)) as a "min-plus" split of the candidate lattice: ONE FP64-pipe instruction per candidate, every one of them
+// independent of the others (no running sum, no dependent chain).
+//
+// The n bits of a candidate b (N = base + b, L123-L127) are split into three groups (low bit j <-> dot n-1-j):
+//     w = bits [0, NW)        u = bits [NW, NL), NL = NU + NW        t = bits [NL, n)  (NH = n - NL of them)
+// One thread owns one high pattern t of one pixel and scores its 2^NL candidates (u, w).  With d0 = base - N_c,
+// h_i = [M d0]_i + 1/2 M_ii (prologue) and h'_j = h_j + sum_{jh in t} M[j][jh], the energy (C1) L607 separates as
+//     e(t,u,w) = A[u] + ( B[w] + QL[u,w] )
+//     B[w]     = offW + sum_{j in w} h'_j                 2^NW values, registers, built once per (thread, pixel)
+//     A[u]     = be + offU + sum_{j in u} h'_j            one DADD per u (prefix sums over the bits of u)
+//     QL[u,w]  = pair energy sum_{j<j' in (u,w)} M_jj'    pixel- and thread-independent: kernel parameter (constant bank)
+//     be       = E(base) + E_C + pairs(t) + sum_{jh in t} h_jh        offW = E_C + sum_{j<NW} |h_j|,  offU = sum_{j>=NW} |h_j|
+// so that  min_w e = A[u] + min_w (B[w] + QL[u,w]):  per candidate ONE DADD  y = B[w] + QL[u,w]  (register + constant
+// operand, static addresses because the loops are fully unrolled) and half an integer min3 on the high words.  The
+// offsets make every y and every A positive, so the high 32 bits of the fp64 pattern order like the values.
+//
+//   qa_minplus_walk_kernel (pass 1; a lower bound per thread):
+//       m_u  = min_w hi32(y)                               (ALU pipe, VIMNMX3)
+//       LB_u = A[u] + double(m_u, 0)   <= min_w e(t,u,w)   (truncation and rounding are monotone)
+//       L_t  = min_u hi32(LB_u)
+//     and, because A[u] > 0, the candidate that attains m_u has e <= A[u] + double(m_u, 0xffffffff), whose high word
+//     is at most hi32(LB_u) + 2.  Hence the thread holding the argmin has L_t <= min_t' L_t' + 2.  Each warp stores
+//     (min of L over its lanes, ballot of lanes with L <= that + 2): 8 bytes.  No barrier, no atomics, no shared memory.
+//   qa_minplus_finish_kernel (pass 2 + S7; one warp per pixel):
+//     survivors = ballot lanes of the warps whose minimum is <= the pixel minimum + 2 (a superset of the threads that can
+//     hold the argmin; normally ONE thread).  Their 2^NL candidates are scored again with pass 1's arithmetic
+//     (same operands, same order, so bitwise the same e) and an exact lexicographic (e, index) compare (reading R6).
+//     The result is therefore exactly the argmin of the pass-1 energies, whose rounding (a few ulp of ~20 E_C) is ten
+//     orders of magnitude below the 1e-9 E_C near-tie rule.  The same warp then decodes N* and recomputes E(N*) from the
+//     definition (S7), so the path is three launches: prologue, walk, finish.
+//
+// FP64-pipe instructions per (thread, pixel): 2^NL (y) + 2*2^NU (A, LB) + 2^NW - 1 (B) + 2 NL (h', offsets) + NH + 1 (be)
+// = 327 per 256 candidates at NU = NW = 4, i.e. 1.28 per candidate (the filtered Gray walk it replaces: 2.06).
+//
+// Index convention as in qa_kernels_walk.cu: candidate index = sum_i b_i 2^(n-1-i) = (t << NL) | (u << NW) | w.
+#include "qa_internal.cuh"
+
+namespace {
+
+constexpr int MP_THREADS = 256;
+constexpr int MF_THREADS = 128;
+
+template <int NL>
+struct alignas(16) MpTable {
+    double q[1 << NL];
+};
+
+__host__ __device__ constexpr int mp_ctz(int k)
+{
+    int j = 0;
+    while (((k >> j) & 1) == 0) ++j;
+    return j;
+}
+
+__device__ __forceinline__ double mp_shfl(double x, int src) { return __shfl_sync(0xffffffffu, x, src); }
+
+// ---- the walk's inner steps, each one asm volatile statement so that the order below (a software pipeline) survives:
+// ptxas places a DADD's consumer right behind it and lets every warp sit out the FP64 latency otherwise.
+// y[k] = b[k] + q[k], k = 0..7: eight independent DADDs
+__device__ __forceinline__ void mp_add8(double (&y)[8], const double (&b)[8], const double (&q)[8])
+{
+    asm volatile(
+        "add.f64 %0, %8, %16; add.f64 %1, %9, %17; add.f64 %2, %10, %18; add.f64 %3, %11, %19;\n"
+        " add.f64 %4, %12, %20; add.f64 %5, %13, %21; add.f64 %6, %14, %22; add.f64 %7, %15, %23;"
+        : "=d"(y[0]), "=d"(y[1]), "=d"(y[2]), "=d"(y[3]), "=d"(y[4]), "=d"(y[5]), "=d"(y[6]), "=d"(y[7])
+        : "d"(b[0]), "d"(b[1]), "d"(b[2]), "d"(b[3]), "d"(b[4]), "d"(b[5]), "d"(b[6]), "d"(b[7]), "d"(q[0]), "d"(q[1]),
+          "d"(q[2]), "d"(q[3]), "d"(q[4]), "d"(q[5]), "d"(q[6]), "d"(q[7]));
+}
+// m0 = min(m0, hi32(y[0..3])), m1 = min(m1, hi32(y[4..7])): four VIMNMX3
+__device__ __forceinline__ void mp_min8(unsigned &m0, unsigned &m1, const double (&y)[8])
+{
+    asm volatile(
+        "{ .reg .b32 lo, h0, h1, h2, h3, h4, h5, h6, h7;\n"
+        " mov.b64 {lo,h0}, %2; mov.b64 {lo,h1}, %3; mov.b64 {lo,h2}, %4; mov.b64 {lo,h3}, %5;\n"
+        " mov.b64 {lo,h4}, %6; mov.b64 {lo,h5}, %7; mov.b64 {lo,h6}, %8; mov.b64 {lo,h7}, %9;\n"
+        " min.u32 h0, h0, h1; min.u32 %0, %0, h0; min.u32 h2, h2, h3; min.u32 %0, %0, h2;\n"
+        " min.u32 h4, h4, h5; min.u32 %1, %1, h4; min.u32 h6, h6, h7; min.u32 %1, %1, h6; }"
+        : "+r"(m0), "+r"(m1)
+        : "d"(y[0]), "d"(y[1]), "d"(y[2]), "d"(y[3]), "d"(y[4]), "d"(y[5]), "d"(y[6]), "d"(y[7]));
+}
+// lb = a + double(m, 0)
+__device__ __forceinline__ void mp_lb(double &lb, double a, unsigned m)
+{
+    asm volatile("{ .reg .f64 z; .reg .b32 zero; mov.b32 zero, 0; mov.b64 z, {zero,%2}; add.f64 %0, %1, z; }"
+                 : "=d"(lb)
+                 : "d"(a), "r"(m));
+}
+// L = min(L, hi32(lb))
+__device__ __forceinline__ void mp_lmin(unsigned &L, double lb)
+{
+    asm volatile("{ .reg .b32 lo, hi; mov.b64 {lo,hi}, %1; min.u32 %0, %0, hi; }" : "+r"(L) : "d"(lb));
+}
+
+// One chunk of the walk: the four u = 4 i + {0..3} against every w, for PX pixels, as a software pipeline over batches of
+// eight DADDs: batch g is issued, then the minima of batch g-1 are taken, then the lower bound of a u whose last batch
+// was g-2 is formed, then that of g-3 enters L.  q = the chunk's 4 * 2^NW table entries; a[ul][px] = A[4 i + ul].
+template <int NW, int PX>
+__device__ __forceinline__ void mp_chunk(const double2 *__restrict__ q, const double (&B)[PX][1 << NW],
+                                         const double (&a)[4][PX], unsigned (&L)[PX])
+{
+    constexpr int EPB = 8 / PX;             // table entries per batch
+    constexpr int BPU = (1 << NW) / EPB;    // batches per u
+    constexpr int G = 4 * BPU;
+    static_assert(PX == 1 || PX == 2, "batches of eight DADDs");
+    double y[2][8], lb[4][PX];
+    unsigned m[4][2];
+#pragma unroll
+    for (int ul = 0; ul < 4; ++ul) m[ul][0] = m[ul][1] = 0xffffffffu;
+#pragma unroll
+    for (int g = 0; g < G + 3; ++g) {
+        if (g < G) {
+            const int ul = g / BPU, w0 = (g % BPU) * EPB;
+            double bb[8], qq[8];
+#pragma unroll
+            for (int k = 0; k < EPB; k += 2) {
+                const double2 t2 = q[((ul << NW) | (w0 + k)) >> 1];
+#pragma unroll
+                for (int px = 0; px < PX; ++px) {
+                    qq[px * EPB + k] = t2.x;
+                    qq[px * EPB + k + 1] = t2.y;
+                    bb[px * EPB + k] = B[px][w0 + k];
+                    bb[px * EPB + k + 1] = B[px][w0 + k + 1];
+                }
+            }
+            mp_add8(y[g & 1], bb, qq);
+        }
+        if (g >= 1 && g <= G) mp_min8(m[(g - 1) / BPU][0], m[(g - 1) / BPU][1], y[(g - 1) & 1]);
+        if (g >= 2 && g - 2 < G && (g - 2) % BPU == BPU - 1) {
+            const int ul = (g - 2) / BPU;
+            if (PX == 2) {
+                mp_lb(lb[ul][0], a[ul][0], m[ul][0]);
+                mp_lb(lb[ul][PX - 1], a[ul][PX - 1], m[ul][1]);
+            } else {
+                mp_lb(lb[ul][0], a[ul][0], min(m[ul][0], m[ul][1]));
+            }
+        }
+        if (g >= 3 && (g - 3) % BPU == BPU - 1) {
+            const int ul = (g - 3) / BPU;
+#pragma unroll
+            for (int px = 0; px < PX; ++px) mp_lmin(L[px], lb[ul][px]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// pass 1.  PX pixels per thread at once: every table entry fetched into a uniform register serves PX DADDs.
+template <int NH, int NU, int NW, int PX, int MINB>
+__global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const QaDevModel *__restrict__ mdl,
+                                                                           const __grid_constant__ MpTable<NU + NW> tab,
+                                                                           QaWorkspace ws)
+{
+    constexpr int NL = NU + NW;
+    constexpr int N = NL + NH;
+    constexpr int TPP = 1 << NH;             // threads per pixel
+    constexpr int WPP = TPP / 32;            // warps per pixel
+    constexpr int SLOTS = MP_THREADS / TPP;  // pixel groups in flight per CTA
+    constexpr int NV = N + 1;                // per-pixel inputs: h[0..N-1], E(base)
+    constexpr int NCH = 1 << (NU - 2);       // chunks of 4 u each
+    static_assert(NH >= 5 && NH <= 8 && N <= 31 && NW >= 2 && NU >= 2, "one or more whole warps per pixel");
+
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned t = threadIdx.x & (TPP - 1);
+    const int slot = threadIdx.x >> NH;
+    const unsigned wq = (threadIdx.x >> 5) % WPP;  // this warp's index among the pixel's warps
+    const int64_t P = ws.P;
+
+    static_assert(NL == QA_WALK_NL, "the model's VT / QHT tables are built for NL = QA_WALK_NL");
+    double v[NL];  // pixel-independent per-thread constants (model tables, qa_api.cu rebuild)
+#pragma unroll
+    for (int j = 0; j < NL; ++j) v[j] = mdl->VT[t * NL + j];
+    const double EC = mdl->EC;
+    const double QH = mdl->QHT[t];
+
+    // Every slot (the TPP threads of one pixel group) is an independent worker; consecutive workers sit in different
+    // CTAs so that a ragged last round is spread over all SMs.
+    const int64_t groups = (P + PX - 1) / PX;
+    const int64_t workers = (int64_t)gridDim.x * SLOTS;
+    const int64_t worker = (int64_t)slot * gridDim.x + blockIdx.x;
+    // lane i < NV of every warp carries input i of the warp's pixel; the next group's is fetched one iteration ahead
+    auto fetch = [&](int64_t grp, int px) -> double {
+        double r = 0.0;
+        if (grp < groups && lane < NV) {
+            int64_t p = grp * PX + px;
+            if (p >= P) p = P - 1;  // ragged last group: the last pixel is walked twice, stored once
+            r = lane < N ? __ldg(ws.h + (int64_t)lane * P + p) : __ldg(ws.e0 + p);
+        }
+        return r;
+    };
+    double nextv[PX];
+#pragma unroll
+    for (int px = 0; px < PX; ++px) nextv[px] = fetch(worker, px);
+
+    for (int64_t grp = worker; grp < groups; grp += workers) {
+        double B[PX][1 << NW];  // B[w]: bits of w added from the highest to the lowest
+        double hu[PX][NU];      // h' of the u bits
+        double a0[PX], lo3[PX];
+#pragma unroll
+        for (int px = 0; px < PX; ++px) {
+            const double myv = nextv[px];
+            nextv[px] = fetch(grp + workers, px);
+            // The offsets must be the same for every thread of the pixel (the L_t are compared across threads), so they
+            // are built from |h_j|, not |h'_j|: h'_j = h_j + v_j(t) >= h_j because M = c_dd^-1 of a Maxwell matrix is >= 0.
+            double hw[NW], offw = EC, offu = 0.0;
+#pragma unroll
+            for (int j = 0; j < NL; ++j) {
+                const double hj = mp_shfl(myv, N - 1 - j);
+                if (j < NW) {
+                    hw[j] = hj + v[j];
+                    offw += fabs(hj);
+                } else {
+                    hu[px][j - NW] = hj + v[j];
+                    offu += fabs(hj);
+                }
+            }
+            double be = mp_shfl(myv, N) + QH;
+#pragma unroll
+            for (int jh = 0; jh < NH; ++jh) {
+                const double hv = mp_shfl(myv, N - 1 - NL - jh);
+                if ((t >> jh) & 1u) be += hv;
+            }
+            a0[px] = be + offu;
+            lo3[px] = hu[px][1] + hu[px][0];
+            B[px][0] = offw;
+#pragma unroll
+            for (int w = 1; w < (1 << NW); ++w) B[px][w] = B[px][w & (w - 1)] + hw[mp_ctz(w)];
+        }
+
+        // A[u] = ah[u >> 2] + lo[u & 3]: ah adds the bits of u >> 2 from the highest down, lo = {0, h'_NW, h'_NW+1, their sum}.
+        // A real loop, one iteration per 4 * 2^NW candidates: the table address is a uniform register plus an immediate
+        // (LDCU UR, c[0x0][UR + imm]) and ptxas schedules one short basic block.  (Fully unrolled it interleaves the chunks,
+        // hoists every table load and spills.)  iv mirrors the loop counter in a vector register the compiler cannot
+        // identify with it: a vector use of the counter itself would turn every table load into a per-thread LDC.
+        unsigned L[PX];
+#pragma unroll
+        for (int px = 0; px < PX; ++px) L[px] = 0xffffffffu;
+        int iv;
+        asm volatile("mov.u32 %0, 0;" : "=r"(iv));
+#pragma unroll 1
+        for (int i = 0; i < NCH; ++i, ++iv) {
+            const double2 *q = reinterpret_cast<const double2 *>(tab.q) + (i << (NW + 1));
+            double a[4][PX];
+#pragma unroll
+            for (int px = 0; px < PX; ++px) {
+                double ah = a0[px];
+#pragma unroll
+                for (int j = NU - 1; j >= 2; --j)
+                    if ((iv >> (j - 2)) & 1) ah += hu[px][j];
+                a[0][px] = ah;
+                a[1][px] = ah + hu[px][0];
+                a[2][px] = ah + hu[px][1];
+                a[3][px] = ah + lo3[px];
+            }
+            mp_chunk<NW, PX>(q, B, a, L);
+        }
+
+#pragma unroll
+        for (int px = 0; px < PX; ++px) {
+            const unsigned wmin = __reduce_min_sync(0xffffffffu, L[px]);
+            const unsigned ball = __ballot_sync(0xffffffffu, L[px] <= wmin + 2u);
+            const int64_t p = grp * PX + px;
+            if (lane == 0 && p < P) ws.rec[p * WPP + wq] = make_uint2(wmin, ball);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// pass 2 + S7: one warp per pixel.  The code runs once per warp (10^4 warps at config 4), so what it pays for is the
+// instruction count and the MIO queue (shuffles, loads), not arithmetic: every lane loads the pixel's inputs itself
+// (warp-uniform addresses, one L1 request each) instead of trading them by shuffle, the survivor's constants come from
+// the model tables, and each lane scores a block of CPL consecutive candidates with a static add tree.
+template <int NH, int NU, int NW>
+__global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaDevModel *__restrict__ mdl,
+                                                                       QaWorkspace ws, int32_t *__restrict__ outN,
+                                                                       double *__restrict__ outE)
+{
+    constexpr int NL = NU + NW;
+    constexpr int N = NL + NH;
+    constexpr int WPP = (1 << NH) / 32;
+    constexpr int LB = NL - 5;          // log2 of the candidates per lane
+    constexpr int CPL = 1 << LB;        // candidates per lane: w = (wb << LB) + c, one u per lane
+    static_assert(LB >= 1 && LB <= NW, "a lane's block of candidates lies inside one u");
+    __shared__ double sd[MF_THREADS / 32][QA_MAXN];
+    __shared__ double sM[N][N];
+    const unsigned lane = threadIdx.x & 31u;
+    const int wid = threadIdx.x >> 5;
+    const int64_t P = ws.P;
+    const int64_t p = (int64_t)blockIdx.x * (MF_THREADS / 32) + wid;
+    const bool live = p < P;
+    const int64_t pp = live ? p : P - 1;
+
+    // Everything that does not depend on the survivor is requested up front, in one round trip: the warp records, the
+    // pixel's inputs (every lane all of them: warp-uniform addresses, one L1 request each), the lane's table entries,
+    // base / N_c of the lane's dot, and M (staged in shared memory for S7).
+    uint2 r = make_uint2(0xffffffffu, 0u);
+    if (lane < WPP) r = ws.rec[pp * WPP + lane];
+    double h[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) h[i] = __ldg(ws.h + (int64_t)i * P + pp);
+    const double e0 = __ldg(ws.e0 + pp);
+    const double EC = mdl->EC;
+    double2 ql[CPL / 2];
+#pragma unroll
+    for (int c = 0; c < CPL / 2; ++c) ql[c] = reinterpret_cast<const double2 *>(mdl->QL + lane * CPL)[c];
+    int32_t base_i = 0;
+    double nc_i = 0.0;
+    if (lane < N) {
+        base_i = ws.base[(int64_t)lane * P + pp];
+        nc_i = ws.nc[(int64_t)lane * P + pp];
+    }
+    for (int e = threadIdx.x; e < N * N; e += MF_THREADS) sM[e / N][e % N] = mdl->M[(e / N) * QA_MAXN + (e % N)];
+    __syncthreads();
+    if (!live) return;
+    const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
+    const unsigned wmask = __ballot_sync(0xffffffffu, lane < WPP && r.x <= H + 2u);  // warps that may hold the argmin
+
+    // thread-independent offsets, as pass 1 formed them (j ascending)
+    double offw = EC, offu = 0.0;
+#pragma unroll
+    for (int j = 0; j < NL; ++j) {
+        if (j < NW)
+            offw += fabs(h[N - 1 - j]);
+        else
+            offu += fabs(h[N - 1 - j]);
+    }
+    const unsigned u = lane >> (NW - LB);                         // this lane's u
+    const unsigned wb = lane & ((1u << (NW - LB)) - 1u);          // ... and the bits of w above its block
+
+    double bestE = INFINITY;
+    unsigned bestI = 0xffffffffu;
+    for (int q = 0; q < WPP; ++q) {
+        unsigned surv = __shfl_sync(0xffffffffu, r.y, q);
+        if (!((wmask >> q) & 1u)) continue;
+        while (surv) {
+            const unsigned ts = (unsigned)q * 32u + (unsigned)(__ffs(surv) - 1);
+            surv &= surv - 1;
+            // the survivor's inputs as pass 1 built them (same operands, same order)
+            double hp[NL];
+#pragma unroll
+            for (int j = 0; j < NL; ++j) hp[j] = h[N - 1 - j] + mdl->VT[ts * NL + j];
+            double be = e0 + mdl->QHT[ts];
+#pragma unroll
+            for (int jh = 0; jh < NH; ++jh)
+                if ((ts >> jh) & 1u) be += h[N - 1 - NL - jh];
+            // A[u] = ah[u >> 2] + lo[u & 3]
+            double a = be + offu;
+#pragma unroll
+            for (int j = NU - 1; j >= 2; --j)
+                if ((u >> j) & 1u) a += hp[NW + j];
+            if ((u & 3u) == 1u) a += hp[NW];
+            if ((u & 3u) == 2u) a += hp[NW + 1];
+            if ((u & 3u) == 3u) a += hp[NW + 1] + hp[NW];
+            // B[w] of the lane's block: bits of w from the highest down
+            double b[CPL];
+            b[0] = offw;
+#pragma unroll
+            for (int j = NW - 1; j >= LB; --j)
+                if ((wb >> (j - LB)) & 1u) b[0] += hp[j];
+#pragma unroll
+            for (int c = 1; c < CPL; ++c) b[c] = b[c & (c - 1)] + hp[mp_ctz(c)];
+            double e1 = INFINITY;
+            unsigned i1 = 0;
+#pragma unroll
+            for (int c = 0; c < CPL; c += 2) {
+                const double ea = a + (b[c] + ql[c >> 1].x), eb = a + (b[c + 1] + ql[c >> 1].y);
+                if (ea < e1) {  // c ascending within the lane: strict '<' keeps the smallest index
+                    e1 = ea;
+                    i1 = c;
+                }
+                if (eb < e1) {
+                    e1 = eb;
+                    i1 = c + 1;
+                }
+            }
+            i1 |= (ts << NL) | (lane << LB);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double e2 = mp_shfl(e1, (int)(lane ^ o));
+                const unsigned i2 = __shfl_xor_sync(0xffffffffu, i1, o);
+                if (e2 < e1 || (e2 == e1 && i2 < i1)) {
+                    e1 = e2;
+                    i1 = i2;
+                }
+            }
+            if (e1 < bestE || (e1 == bestE && i1 < bestI)) {
+                bestE = e1;
+                bestI = i1;
+            }
+        }
+    }
+    if (!outN) {
+        if (lane == 0) ws.best[p] = (uint64_t)bestI;
+        return;
+    }
+    // S7: N* and E(N*) = 1/2 d^T M d from the definition (Eq. (C1)); lane i holds dot i, d goes through shared memory
+    int32_t Ni = 0;
+    double di = 0.0;
+    if (lane < N) {
+        Ni = base_i + (int32_t)((bestI >> (N - 1 - lane)) & 1u);
+        di = (double)Ni - nc_i;
+        sd[wid][lane] = di;
+    }
+    __syncwarp();
+    const int li = lane < N ? lane : 0;
+    double row = 0.0;
+#pragma unroll
+    for (int j = 0; j < N; ++j) row = fma(sM[li][j], sd[wid][j], row);
+    double E = di * row;  // lanes >= N hold di = 0
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) E += mp_shfl(E, (int)(lane ^ o));
+    if (lane < N) outN[p * N + lane] = Ni;
+    if (lane == 0) outE[p] = 0.5 * E;
+}
+
+template <int NH, int NU, int NW, int PX, int MINB>
+cudaError_t launch_mp(const QaDevModel *d_model, const double *QLhost, QaWorkspace ws, int32_t *d_N, double *d_E,
+                      int sm_count, cudaStream_t stream)
+{
+    constexpr int NL = NU + NW;
+    constexpr int SLOTS = MP_THREADS >> NH;
+    MpTable<NL> local;  // the first 2^NL entries of the model's table (the table of fewer low bits is a prefix)
+    for (int b = 0; b < (1 << NL); ++b) local.q[b] = QLhost[b];
+    int per_sm = 0;
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_walk_kernel<NH, NU, NW, PX, MINB>,
+                                                                    MP_THREADS, 0);
+    if (err != cudaSuccess) return err;
+    if (per_sm < 1) per_sm = 1;
+    int64_t grid = (int64_t)sm_count * per_sm;
+    const int64_t need = ((ws.P + PX - 1) / PX + SLOTS - 1) / SLOTS;
+    if (grid > need) grid = need;
+    qa_minplus_walk_kernel<NH, NU, NW, PX, MINB><<<(unsigned)grid, MP_THREADS, 0, stream>>>(d_model, local, ws);
+    err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
+    qa_plan_add("qa_minplus_finish_kernel");
+    qa_timing_mark(stream);
+    const int64_t fblocks = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
+    qa_minplus_finish_kernel<NH, NU, NW><<<(unsigned)fblocks, MF_THREADS, 0, stream>>>(d_model, ws, d_N, d_E);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// d_N == nullptr: the finish kernel only stores the winning index (ws.best) and the caller runs qa_finalize_kernel.
+cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
+                                   double *d_E, int sm_count, cudaStream_t stream)
+{
+    qa_plan_add("qa_minplus_walk_kernel");
+#define MP_CALL(NH) launch_mp<NH, 4, 4, 2, 2>(d_model, QLhost, ws, d_N, d_E, sm_count, stream)
+    switch (n) {
+        case 13: return MP_CALL(5);
+        case 14: return MP_CALL(6);
+        case 15: return MP_CALL(7);
+        case 16: return MP_CALL(8);
+        default: return cudaErrorInvalidValue;
+    }
+#undef MP_CALL
+}

@@ -97,30 +97,45 @@ def test_config4_open_grid16_default(api, W, H):
     """n = 16, 2^16 candidates per pixel: the hot kernel (NL = 8, NH = 8), QP pixels included."""
     w = wl.config4(W, H)
     rep, g, o = check(api, w, algorithm="default")
-    assert g["plan"][0] == ["qa_prologue_kernel", "qa_filter_walk_kernel", "qa_filter_finish_kernel"]
+    assert g["plan"][0] == ["qa_prologue_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"]
     assert g["stats"]["n_candidates_scored"] == w.P * 65536
 
 
-@pytest.mark.parametrize("n", [13, 14, 16])
-def test_walk_variants_agree(api, n):
-    """The exact-compare walk, the filtered walk with a separate finalize and the fused filtered walk give the same
-    charge map and the same energies up to the summation order of E(N*); each is also checked against the oracle."""
-    w = wl.random_open(n, n, 45, seed=200 + n)
+@pytest.mark.parametrize("n,P", [(13, 45), (14, 46), (15, 33), (16, 45), (16, 1)])
+def test_walk_variants_agree(api, n, P):
+    """The exact-compare Gray walk (variant 0) and the min-plus walk + finish kernel (variant 1, the default for
+    n >= 13) give the same charge map and the same energies up to the summation order of E(N*); each is also checked
+    against the oracle.  P odd / P = 1: the ragged last pixel pair of the min-plus walk."""
+    w = wl.random_open(n, n, P, seed=200 + n)
     ref = None
     try:
-        for variant in (0, 1, 2, 3):
+        for variant in (0, 1):
             api.set_walk_variant(variant)
             rep, g, o = check(api, w, algorithm="default")
             names = g["plan"][0]
-            assert names[1] == ("qa_walk_kernel" if variant == 0 else "qa_filter_walk_kernel")
-            assert len(names) == {0: 3, 1: 4, 2: 3, 3: 3}[variant]
+            assert names == (["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"] if variant == 0 else
+                             ["qa_prologue_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"])
             if ref is None:
                 ref = g
             else:
                 assert np.array_equal(ref["N"], g["N"])
                 assert np.allclose(ref["E"], g["E"], rtol=1e-13, atol=1e-13 * g["EC"])
     finally:
-        api.set_walk_variant(2)
+        api.set_walk_variant(1)
+
+
+def test_minplus_walk_extreme_inputs(api):
+    """Pixels far outside the operating range: every dot clamped (N_c << 0, huge positive h) and large occupations."""
+    w = wl.config4(6, 5)
+    rng = np.random.default_rng(7)
+    Vg = np.concatenate([w.Vg, -50.0 * np.abs(rng.standard_normal((7, 16))), w.Vg[:9] * 40.0, np.zeros((3, 16))])
+    w.Vg, w.W, w.H = np.ascontiguousarray(Vg), Vg.shape[0], 1
+    try:
+        for variant in (0, 1):
+            api.set_walk_variant(variant)
+            check(api, w, algorithm="default")
+    finally:
+        api.set_walk_variant(1)
 
 
 def test_config5_open_grid8_default_and_thresholded(api):
