@@ -87,6 +87,30 @@ cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int it
 
 // ---- small device helpers ------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
+// Programmatic dependent launch (sm_90+): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may
+// become resident while its predecessor in the stream is still running; it must call qa_pdl_wait() before it touches
+// anything the predecessor wrote (the wait returns once that grid has completed and its writes are visible).
+// qa_pdl_launch_dependents() lets the successor's CTAs be scheduled as soon as resources free up.
+__device__ __forceinline__ void qa_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void qa_pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// Launch `kernel` as a programmatic dependent of the previous kernel in `stream`.
+template <typename... KArgs, typename... Args>
+inline cudaError_t qa_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 __device__ __forceinline__ void qa_atomic_add64(int64_t *addr, int64_t v)
 {
     atomicAdd(reinterpret_cast<unsigned long long *>(addr), static_cast<unsigned long long>(v));

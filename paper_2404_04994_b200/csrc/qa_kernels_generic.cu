@@ -159,6 +159,7 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
     if (threadIdx.x < N) sC1[threadIdx.x] = mdl->C1[threadIdx.x];
     const double oneC1 = mdl->oneC1;
     __syncthreads();
+    qa_pdl_launch_dependents();  // the candidate kernel may become resident and load its constants meanwhile
 
     const int64_t P = ws.P;
     const int64_t p = blockIdx.x * (int64_t)PRO_THREADS + threadIdx.x;

@@ -187,6 +187,8 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
         }
         return r;
     };
+    qa_pdl_launch_dependents();
+    qa_pdl_wait();  // everything above reads model constants only; h / e0 come from the prologue kernel
     double nextv[PX];
 #pragma unroll
     for (int px = 0; px < PX; ++px) nextv[px] = fetch(worker, px);
@@ -292,23 +294,24 @@ __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaD
     // Everything that does not depend on the survivor is requested up front, in one round trip: the warp records, the
     // pixel's inputs (every lane all of them: warp-uniform addresses, one L1 request each), the lane's table entries,
     // base / N_c of the lane's dot, and M (staged in shared memory for S7).
+    const double EC = mdl->EC;
+    double2 ql[CPL / 2];
+#pragma unroll
+    for (int c = 0; c < CPL / 2; ++c) ql[c] = reinterpret_cast<const double2 *>(mdl->QL + lane * CPL)[c];
+    for (int e = threadIdx.x; e < N * N; e += MF_THREADS) sM[e / N][e % N] = mdl->M[(e / N) * QA_MAXN + (e % N)];
+    qa_pdl_wait();  // model constants above; everything below was written by the prologue / walk kernels
     uint2 r = make_uint2(0xffffffffu, 0u);
     if (lane < WPP) r = ws.rec[pp * WPP + lane];
     double h[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) h[i] = __ldg(ws.h + (int64_t)i * P + pp);
     const double e0 = __ldg(ws.e0 + pp);
-    const double EC = mdl->EC;
-    double2 ql[CPL / 2];
-#pragma unroll
-    for (int c = 0; c < CPL / 2; ++c) ql[c] = reinterpret_cast<const double2 *>(mdl->QL + lane * CPL)[c];
     int32_t base_i = 0;
     double nc_i = 0.0;
     if (lane < N) {
         base_i = ws.base[(int64_t)lane * P + pp];
         nc_i = ws.nc[(int64_t)lane * P + pp];
     }
-    for (int e = threadIdx.x; e < N * N; e += MF_THREADS) sM[e / N][e % N] = mdl->M[(e / N) * QA_MAXN + (e % N)];
     __syncthreads();
     if (!live) return;
     const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
@@ -428,14 +431,14 @@ cudaError_t launch_mp(const QaDevModel *d_model, const double *QLhost, QaWorkspa
     int64_t grid = (int64_t)sm_count * per_sm;
     const int64_t need = ((ws.P + PX - 1) / PX + SLOTS - 1) / SLOTS;
     if (grid > need) grid = need;
-    qa_minplus_walk_kernel<NH, NU, NW, PX, MINB><<<(unsigned)grid, MP_THREADS, 0, stream>>>(d_model, local, ws);
-    err = cudaGetLastError();
+    err = qa_launch_pdl(qa_minplus_walk_kernel<NH, NU, NW, PX, MINB>, dim3((unsigned)grid), dim3(MP_THREADS), stream, d_model,
+                        local, ws);
     if (err != cudaSuccess) return err;
     qa_plan_add("qa_minplus_finish_kernel");
     qa_timing_mark(stream);
     const int64_t fblocks = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
-    qa_minplus_finish_kernel<NH, NU, NW><<<(unsigned)fblocks, MF_THREADS, 0, stream>>>(d_model, ws, d_N, d_E);
-    return cudaGetLastError();
+    return qa_launch_pdl(qa_minplus_finish_kernel<NH, NU, NW>, dim3((unsigned)fblocks), dim3(MF_THREADS), stream, d_model, ws,
+                         d_N, d_E);
 }
 
 }  // namespace
