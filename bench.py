@@ -29,6 +29,7 @@ import numpy as np  # noqa: E402
 METRIC = "candidate configs scored/s (16 dots, default algorithm, open 4x4 grid, 100x100 pixels)"
 UNIT = "candidates/s"
 FP64_OPS_PER_CANDIDATE = 334.0 / 256.0   # FP64-pipe instructions per candidate of the min-plus walk
+WALK_DRAM_BYTES_NCU = 1392384           # profiles/r01_walk_kernel_ncu_full.md: dram__bytes_read + dram__bytes_write per launch
 FP64_LANES_PER_SM = 64         # 148 SMs x 64 FP64 lanes x SM clock
 
 
@@ -230,7 +231,8 @@ def run_ours(args, rank, world, local_rank):
     alg_ops = ops_per_cand * wls[0].P * (2 ** wls[0].n_dot)
     achieved = alg_ops / (walk_ms * 1e-3) if walk_ms > 0 else 0.0
     roofline = {"bound": "alu", "kernel": hot, "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
-                "unit": "FP64 Ginst/s", "frac": achieved / peak_nominal, "traffic": None,
+                "unit": "FP64 Ginst/s", "frac": achieved / peak_nominal,
+                "traffic": WALK_DRAM_BYTES_NCU if hot == "qa_minplus_walk_kernel" else None, "traffic_unit": "bytes/launch (ncu dram read+write)",
                 "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max_mhz:.0f} MHz "
                                "(DESIGN.md); MEASURED_PEAKS.json has no FP64 figure",
                 "peak_measured_dfma_probe": peak_measured / 1e9, "frac_of_measured_probe": achieved / peak_measured,

@@ -124,9 +124,10 @@ QA_API qa_status qa_ground_state_closed(const qa_model *model, const double *d_V
                                  qa_stats *d_stats, void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 
 /* Host-buffer convenience (the end-to-end path): same semantics with HOST pointers.  Copies V_g to the device, runs the
- * search, copies the results back and synchronises before returning.  Device scratch comes from the stream-ordered pool
- * (cudaMallocAsync) and is released before return.  closed = 0/1; N_hat is ignored for open arrays.  h_stats may be
- * NULL; it is overwritten, not accumulated. */
+ * search, copies the results back and synchronises before returning.  The model keeps a private stream and a grow-only
+ * device staging buffer for these calls (released by qa_model_destroy); concurrent host calls on one model serialise.
+ * closed = 0/1; N_hat is ignored for open arrays.  h_stats may be NULL; it is overwritten, not accumulated.  Pinned
+ * host buffers make the copies asynchronous DMA transfers; pageable ones work too. */
 QA_API qa_status qa_ground_state_host(const qa_model *model, const double *h_Vg, int64_t P, int closed, int N_hat,
                                qa_algorithm alg, double t, int n_max, int32_t *h_N, double *h_E, double *h_xcont,
                                double *h_Vsensor, qa_stats *h_stats);

@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -22,6 +23,12 @@ struct qa_model {
     QaDevModel host;        // mirror of the device constants
     QaDevModel *dev;        // device copy
     QaWalkTable walk;       // pair table of the low bits of the search model
+    // qa_ground_state_host: a private stream and a grow-only device staging buffer, reused from call to call (creating
+    // a stream and going through the allocator cost more than the search itself on a 100x100 diagram)
+    std::mutex host_mu;
+    cudaStream_t host_stream;
+    char *host_buf;
+    size_t host_buf_bytes;
 };
 
 namespace {
@@ -289,9 +296,8 @@ qa_status qa_model_create(const double *C_dd, const double *C_gd, int n_dot, int
             if (std::fabs(C_dd[i * n_dot + j] - C_dd[j * n_dot + i]) > 1e-12 * amax) return QA_ERR_NOT_SYMMETRIC;
             if (C_dd[i * n_dot + j] > 0.0) is_z = false;
         }
-    qa_model *m = new (std::nothrow) qa_model;
+    qa_model *m = new (std::nothrow) qa_model();  // value-initialised: every plain member zero
     if (!m) return QA_ERR_INVALID_ARG;
-    std::memset(static_cast<void *>(m), 0, sizeof(*m));
     m->nf = n_dot;
     m->g = n_gate;
     m->ns = 0;
@@ -347,6 +353,8 @@ qa_status qa_model_destroy(qa_model *m)
 {
     if (!m) return QA_OK;
     cudaError_t e = cudaFree(m->dev);
+    if (m->host_buf) cudaFree(m->host_buf);
+    if (m->host_stream) cudaStreamDestroy(m->host_stream);
     delete m;
     return e == cudaSuccess ? QA_OK : cuda_fail(e, "qa_model_destroy");
 }
@@ -386,25 +394,30 @@ qa_status qa_ground_state_closed(const qa_model *m, const double *d_Vg, int64_t 
                         workspace_bytes, cuda_stream);
 }
 
-qa_status qa_ground_state_host(const qa_model *m, const double *h_Vg, int64_t P, int closed, int N_hat, qa_algorithm alg,
+qa_status qa_ground_state_host(const qa_model *mc, const double *h_Vg, int64_t P, int closed, int N_hat, qa_algorithm alg,
                                double t, int n_max, int32_t *h_N, double *h_E, double *h_xcont, double *h_Vsensor,
                                qa_stats *h_stats)
 {
-    if (!m || P < 0 || (P > 0 && (!h_Vg || !h_N || !h_E))) return QA_ERR_INVALID_ARG;
+    if (!mc || P < 0 || (P > 0 && (!h_Vg || !h_N || !h_E))) return QA_ERR_INVALID_ARG;
     if (P == 0) return QA_OK;
+    qa_model *m = const_cast<qa_model *>(mc);  // only the host-call staging state below is touched, under its mutex
+    std::lock_guard<std::mutex> lock(m->host_mu);
     const size_t Pz = (size_t)P, nf = (size_t)m->nf, n = (size_t)m->host.n, g = (size_t)m->g, ns = (size_t)m->ns;
     const size_t bVg = align256(Pz * g * 8), bN = align256(Pz * nf * 4), bE = align256(Pz * 8);
     const size_t bX = h_xcont ? align256(Pz * n * 8) : 0, bVs = (h_Vsensor && ns) ? align256(Pz * ns * 8) : 0;
     const size_t bS = h_stats ? align256(sizeof(qa_stats)) : 0, bW = qa_workspace_bytes(m, P);
-    cudaStream_t stream = nullptr;
-    char *buf = nullptr;
-    QA_CUDA(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
-    qa_status st = QA_OK;
-    cudaError_t e = cudaMallocAsync(reinterpret_cast<void **>(&buf), bVg + bN + bE + bX + bVs + bS + bW, stream);
-    if (e != cudaSuccess) {
-        cudaStreamDestroy(stream);
-        return cuda_fail(e, "cudaMallocAsync");
+    const size_t need = bVg + bN + bE + bX + bVs + bS + bW;
+    if (!m->host_stream) QA_CUDA(cudaStreamCreateWithFlags(&m->host_stream, cudaStreamNonBlocking));
+    cudaStream_t stream = m->host_stream;
+    if (m->host_buf_bytes < need) {
+        if (m->host_buf) QA_CUDA(cudaFree(m->host_buf));
+        m->host_buf = nullptr;
+        m->host_buf_bytes = 0;
+        QA_CUDA(cudaMalloc(reinterpret_cast<void **>(&m->host_buf), need));
+        m->host_buf_bytes = need;
     }
+    char *buf = m->host_buf;
+    qa_status st = QA_OK;
     double *dVg = reinterpret_cast<double *>(buf);
     int32_t *dN = reinterpret_cast<int32_t *>(buf + bVg);
     double *dE = reinterpret_cast<double *>(buf + bVg + bN);
@@ -412,7 +425,7 @@ qa_status qa_ground_state_host(const qa_model *m, const double *h_Vg, int64_t P,
     double *dVs = bVs ? reinterpret_cast<double *>(buf + bVg + bN + bE + bX) : nullptr;
     qa_stats *dS = bS ? reinterpret_cast<qa_stats *>(buf + bVg + bN + bE + bX + bVs) : nullptr;
     void *dW = buf + bVg + bN + bE + bX + bVs + bS;
-    e = cudaMemcpyAsync(dVg, h_Vg, Pz * g * 8, cudaMemcpyHostToDevice, stream);
+    cudaError_t e = cudaMemcpyAsync(dVg, h_Vg, Pz * g * 8, cudaMemcpyHostToDevice, stream);
     if (e == cudaSuccess && dS) e = cudaMemsetAsync(dS, 0, sizeof(qa_stats), stream);
     if (e == cudaSuccess) {
         st = ground_state(m, dVg, P, closed, N_hat, alg, t, n_max, dN, dE, dX, dVs, dS, dW, bW, stream);
@@ -426,9 +439,7 @@ qa_status qa_ground_state_host(const qa_model *m, const double *h_Vg, int64_t P,
                 e = cudaMemcpyAsync(h_stats, dS, sizeof(qa_stats), cudaMemcpyDeviceToHost, stream);
         }
     }
-    cudaFreeAsync(buf, stream);
     cudaError_t e2 = cudaStreamSynchronize(stream);
-    cudaStreamDestroy(stream);
     if (st != QA_OK) return st;
     if (e != cudaSuccess) return cuda_fail(e, "qa_ground_state_host");
     if (e2 != cudaSuccess) return cuda_fail(e2, "qa_ground_state_host sync");
