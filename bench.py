@@ -42,6 +42,8 @@ def parse():
     ap.add_argument("--workload", default="config4", choices=["config4", "config5"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--arrays", type=int, default=256, help="config5: arrays of the dataset batch per GPU")
+    ap.add_argument("--streams", type=int, default=8, help="config5: CUDA streams the independent calls are spread over")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -279,6 +281,106 @@ def run_ours(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------------------------------
+def run_config5(args, rank, world, local_rank):
+    """Secondary workload (BASELINE.json configs[4]): the dataset batch of independently seeded open 8-dot arrays, each a
+    128x128 sweep, with the default algorithm and the thresholded one at t = 0.2 and 0.5.  One step = every array with
+    all three algorithms.  Arrays are independent calls of the single-model entry point, spread round-robin over a few
+    CUDA streams (each call is less than one wave of the GPU).  Reports pixels/s over the whole batch and the
+    agreement rate of thresholded vs default (fraction of pixels with identical N)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2404_04994_b200 import api, workloads as wl
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    B = args.arrays
+    wls = [wl.config5_array(j + B * rank) for j in range(B)]
+    models = [api.Model(w.C_dd, w.C_gd) for w in wls]
+    Vgs = [torch.from_numpy(w.Vg).to(dev) for w in wls]
+    algs = (("default", dict(algorithm="default")), ("t0.2", dict(algorithm="thresholded", t=0.2)),
+            ("t0.5", dict(algorithm="thresholded", t=0.5)))
+    outs = {a: [{"N": torch.empty((w.P, w.n_dot), dtype=torch.int32, device=dev),
+                 "E": torch.empty(w.P, dtype=torch.float64, device=dev)} for w in wls] for a, _ in algs}
+    # one model object per (array, algorithm): a model owns its workspace, and the three calls of an array may overlap
+    mods = {a: ([api.Model(w.C_dd, w.C_gd) for w in wls] if a != "default" else models) for a, _ in algs}
+    streams = [torch.cuda.Stream(dev) for _ in range(args.streams)]
+    px_step = sum(w.P for w in wls) * len(algs)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        cur = torch.cuda.current_stream(dev)
+        for s_ in streams:
+            s_.wait_stream(cur)
+        k = 0
+        for a, kw in algs:
+            for j in range(B):
+                s_ = streams[k % len(streams)]
+                k += 1
+                with torch.cuda.stream(s_):
+                    mods[a][j].ground_state(Vgs[j], out=outs[a][j], **kw)
+        for s_ in streams:
+            cur.wait_stream(s_)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        flush.fill_(1)
+        step()
+    launches_per_step = api.last_launch_plan()[1] * B * len(algs)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)
+        ev[k][0].record()
+        step()
+        ev[k][1].record()
+    barrier()
+    clocks = sampler.stop()
+    times = np.array([a.elapsed_time(b) for a, b in ev])
+    tot_ms = float(times.sum())
+    if world > 1:
+        tt = torch.tensor([tot_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        tot_ms = float(tt.item())
+    ms_per_step = tot_ms / args.steps
+    if rank != 0:
+        return
+    agree = {}
+    for a in ("t0.2", "t0.5"):
+        same = sum(int((outs[a][j]["N"] == outs["default"][j]["N"]).all(dim=1).sum()) for j in range(B))
+        agree[a] = same / (px_step / len(algs))
+    n, g = wls[0].n_dot, wls[0].n_gate
+    bytes_px = 8 * g + 4 * n + 8                       # DESIGN.md section 6: V_g in, N and E out
+    hbm = None
+    try:
+        hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        pass
+    peak = hbm or 6516.0
+    achieved = px_step * bytes_px / (ms_per_step * 1e-3) / 1e9
+    line = {"metric": "pixels/s over the dataset batch (open 8-dot arrays, 128x128, default + thresholded t=0.2, 0.5)",
+            "value": world * px_step / (ms_per_step * 1e-3), "unit": "pixels/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[4]: {B} open 8-dot arrays (seeds 1000+j), 128x128 each, "
+                                   "default + thresholded t=0.2 + t=0.5", "arrays_per_gpu": B, "streams": len(streams),
+                       "pixels_per_step_per_gpu": px_step, "l2": "flushed (256 MiB write) between timed steps",
+                       "parallelism": f"array-range x{world}"},
+            "agreement_with_default": agree,
+            "roofline": {"bound": "hbm", "kernel": "whole step (prologue + walk/enumerate + finalize per call)",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "bytes_per_pixel": bytes_px,
+                         "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm else "fallback 6516 GB/s (SURVEY.md)"},
+            "cpu_baseline": None, "e2e": None, "gpu_launches": launches_per_step * args.steps, "clocks": clocks}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0"))
@@ -296,7 +398,10 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl")
         dist.barrier()
-    run_ours(args, rank, world, local_rank)
+    if args.workload == "config5":
+        run_config5(args, rank, world, local_rank)
+    else:
+        run_ours(args, rank, world, local_rank)
     if world > 1:
         import torch.distributed as dist
         dist.barrier()

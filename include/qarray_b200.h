@@ -48,8 +48,7 @@ typedef enum {
     QA_ERR_INFEASIBLE = 5,       /* closed array: N_hat < 0, or brute force with n_dot * n_max < N_hat                 */
     QA_ERR_OVERFLOW = 6,         /* brute force: (n_max + 1)^n_dot >= 2^62                                             */
     QA_ERR_CUDA = 7,             /* a CUDA runtime call failed; see qa_last_cuda_error()                               */
-    QA_ERR_UNSUPPORTED = 8       /* c_dd has a positive off-diagonal entry (not a Maxwell matrix, L35): the exact
-                                    clamp-only QP of reading R3 needs offdiag <= 0                                     */
+    QA_ERR_UNSUPPORTED = 8       /* reserved (earlier versions refused a c_dd with a positive off-diagonal entry)      */
 } qa_status;
 
 /* The three candidate sets of the paper (Table I). */
@@ -74,8 +73,10 @@ typedef struct {
 /* ---- model ------------------------------------------------------------------------------------------------------- */
 
 /* Problem statement: the constructor of the paper's DotArray (L185-L201) with Maxwell-format inputs.
- * C_dd : host, [n_dot*n_dot], symmetric positive definite, off-diagonals <= 0 (L35, Eq. (B1)).  Validated as in
- *        L204: finite, symmetric (QA_ERR_NOT_SYMMETRIC), positive definite (QA_ERR_NOT_POSDEF).
+ * C_dd : host, [n_dot*n_dot], symmetric positive definite; a Maxwell matrix has off-diagonals <= 0 (L35, Eq. (B1)).
+ *        Validated as in L204: finite, symmetric (QA_ERR_NOT_SYMMETRIC), positive definite (QA_ERR_NOT_POSDEF).  A
+ *        positive off-diagonal entry is legal input: the continuous QP then runs its general active-set phase and the
+ *        open default search of n_dot >= 13 uses the exact-compare walk (reading R3).
  * C_gd : host, [n_dot*n_gate], gate->dot couplings (positive convention, reading on L35 vs L90).
  * Computes M = c_dd^-1, c_dd 1, 1^T c_dd 1 (Eq. (7)) and the pixel-independent pair-energy tables on the host, and
  * uploads them to the CURRENT CUDA device.  *out is owned by the library until qa_model_destroy. */

@@ -228,7 +228,6 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
         if (std::pow((double)n_max + 1.0, (double)n) >= 4.611686018427388e18) return QA_ERR_OVERFLOW;
         if (closed && (int64_t)n * n_max < N_hat) return QA_ERR_INFEASIBLE;
     }
-    if (!m->is_z) return QA_ERR_UNSUPPORTED;
     if (P == 0) return QA_OK;
     if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
     if (!d_ws || ws_bytes < carve(m, P, nullptr, nullptr) || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
@@ -236,12 +235,13 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     QaWorkspace ws;
     carve(m, P, d_ws, &ws);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    QaCallArgs a{closed, N_hat, (int)alg, t, n_max};
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1};
     g_n_marks = 0;
     timing_mark(stream);
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
     timing_mark(stream);
-    if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && walk_variant() != 0) {
+    // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd
+    if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && walk_variant() != 0 && m->is_z) {
         const bool fuse = m->ns == 0;  // S7 runs inside the finish kernel: no finalize launch
         QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count, stream));
         timing_mark(stream);
@@ -527,7 +527,7 @@ const char *qa_status_string(qa_status s)
         case QA_ERR_INFEASIBLE: return "closed array: no admissible charge state";
         case QA_ERR_OVERFLOW: return "brute force: (n_max+1)^n_dot >= 2^62";
         case QA_ERR_CUDA: return "CUDA error";
-        case QA_ERR_UNSUPPORTED: return "c_dd has a positive off-diagonal entry (not a Maxwell matrix)";
+        case QA_ERR_UNSUPPORTED: return "unsupported (reserved; not returned by this version)";
     }
     return "unknown status";
 }

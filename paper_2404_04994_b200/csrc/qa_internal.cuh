@@ -59,6 +59,7 @@ struct QaCallArgs {
     int alg;
     double t;
     int n_max;
+    int general_qp;  // c_dd has a positive off-diagonal: the QP continues with the primal active-set phase (R3)
 };
 
 // Pair-energy table of the low QA_WALK_NL bits for the static walk: QL[b] = sum_{j<j', both set in b} M[a_j][a_j'],

@@ -22,9 +22,92 @@ constexpr int FIN_THREADS = 128;
 //   closed: y_A = a - lambda b,  a = -C_AA^-1 c_A,  b = C_AA^-1 C_AF 1_F,
 //           lambda = (N_hat - sum c_F - 1^T C_FA a) / (1^T C_FF 1 - 1^T C_FA b),  x_F = c_F + C_FA y_A + lambda C_FF 1_F
 // Multipliers of the bounds: r_A = y_A - lambda >= 0 is verified (KKT); a violation is counted in n_qp_failed.
+// Minimiser of the objective with the dots of A held at 0 (and, closed, 1^T x = N_hat): xe, and the multipliers of the
+// held bounds r_i = y_i - lambda, i in A (r of a free dot is 0).  0 < |A| < N.
 template <int N>
-__device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool closed, double Nhat, double *x,
-                           bool &failed)
+__device__ void qa_qp_eqp(const double *__restrict__ sC, const double *c, bool closed, double Nhat, unsigned A, double *xe,
+                          double *r)
+{
+    int ia[N], k = 0;
+    for (int i = 0; i < N; ++i)
+        if ((A >> i) & 1u) ia[k++] = i;
+    // Cholesky C_AA = L L^T
+    double L[N * N], a[N], b[N], rb[N];
+    for (int p = 0; p < k; ++p) {
+        for (int q = 0; q <= p; ++q) {
+            double s = sC[ia[p] * N + ia[q]];
+            for (int t = 0; t < q; ++t) s -= L[p * N + t] * L[q * N + t];
+            if (p == q)
+                L[p * N + p] = sqrt(s);
+            else
+                L[p * N + q] = s / L[q * N + q];
+        }
+    }
+    auto solve = [&](const double *rhs, double *out) {
+        for (int p = 0; p < k; ++p) {
+            double s = rhs[p];
+            for (int t = 0; t < p; ++t) s -= L[p * N + t] * out[t];
+            out[p] = s / L[p * N + p];
+        }
+        for (int p = k - 1; p >= 0; --p) {
+            double s = out[p];
+            for (int t = p + 1; t < k; ++t) s -= L[t * N + p] * out[t];
+            out[p] = s / L[p * N + p];
+        }
+    };
+    for (int q = 0; q < k; ++q) rb[q] = -c[ia[q]];
+    solve(rb, a);
+    double lam = 0.0;
+    if (closed) {
+        double sumcF = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+        for (int q = 0; q < k; ++q) {
+            double s = 0.0;
+            for (int f = 0; f < N; ++f)
+                if (!((A >> f) & 1u)) s += sC[ia[q] * N + f];
+            rb[q] = s;
+        }
+        solve(rb, b);
+        for (int f = 0; f < N; ++f) {
+            if ((A >> f) & 1u) continue;
+            sumcF += c[f];
+            for (int q = 0; q < k; ++q) {
+                t1 += sC[f * N + ia[q]] * a[q];
+                t3 += sC[f * N + ia[q]] * b[q];
+            }
+            for (int f2 = 0; f2 < N; ++f2)
+                if (!((A >> f2) & 1u)) t2 += sC[f * N + f2];
+        }
+        lam = (Nhat - sumcF - t1) / (t2 - t3);
+        for (int q = 0; q < k; ++q) a[q] -= lam * b[q];
+    }
+    for (int f = 0; f < N; ++f) r[f] = 0.0;
+    for (int q = 0; q < k; ++q) r[ia[q]] = a[q] - lam;
+    for (int f = 0; f < N; ++f) {
+        if ((A >> f) & 1u) {
+            xe[f] = 0.0;  // clamped components are exactly 0 (R3)
+            continue;
+        }
+        double s = c[f];
+        for (int q = 0; q < k; ++q) s += sC[f * N + ia[q]] * a[q];
+        if (closed) {
+            double rowF = 0.0;
+            for (int f2 = 0; f2 < N; ++f2)
+                if (!((A >> f2) & 1u)) rowF += sC[f * N + f2];
+            s += lam * rowF;
+            if (k == N - 1) s = Nhat;  // R3: a single free dot carries the whole charge, exactly
+        }
+        xe[f] = s;
+    }
+}
+
+// Phase 1 (every c_dd): the monotone clamp-only active set described above.  For a Maxwell c_dd it ends at the KKT point.
+// Phase 2 (only when c_dd has a positive off-diagonal, `general`): phase 1 still ends at a feasible x that minimises the
+// objective on its face x_A = 0, but a bound multiplier may be negative; from there the textbook primal active-set method
+// continues (release the most negative multiplier, move towards the new face minimiser, stop at the first bound that
+// blocks), which terminates at the unique KKT point of the strictly convex problem.
+template <int N>
+__device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool closed, double Nhat, bool general,
+                           double *x, bool &failed)
 {
     unsigned A = 0;
     int rounds = 0;
@@ -34,6 +117,8 @@ __device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool 
         for (int i = 0; i < N; ++i) x[i] = 0.0;
         return 1;
     }
+    double r[N];
+    for (int i = 0; i < N; ++i) r[i] = 0.0;
     for (;;) {
         unsigned neg = 0;
         for (int i = 0; i < N; ++i)
@@ -45,82 +130,79 @@ __device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool 
             failed = true;
             break;
         }
-        int ia[N], k = 0;
-        for (int i = 0; i < N; ++i)
-            if ((A >> i) & 1u) ia[k++] = i;
-        if (k == N) {  // nothing left free: only consistent for an open array
+        if (__popc(A) == N) {  // nothing left free: only consistent for an open array
             for (int i = 0; i < N; ++i) x[i] = 0.0;
             if (closed) failed = true;
             break;
         }
-        // Cholesky C_AA = L L^T
-        double L[N * N], a[N], b[N], rb[N];
-        for (int p = 0; p < k; ++p) {
-            for (int q = 0; q <= p; ++q) {
-                double s = sC[ia[p] * N + ia[q]];
-                for (int r = 0; r < q; ++r) s -= L[p * N + r] * L[q * N + r];
-                if (p == q)
-                    L[p * N + p] = sqrt(s);
-                else
-                    L[p * N + q] = s / L[q * N + q];
-            }
-        }
-        auto solve = [&](const double *rhs, double *out) {
-            for (int p = 0; p < k; ++p) {
-                double s = rhs[p];
-                for (int r = 0; r < p; ++r) s -= L[p * N + r] * out[r];
-                out[p] = s / L[p * N + p];
-            }
-            for (int p = k - 1; p >= 0; --p) {
-                double s = out[p];
-                for (int r = p + 1; r < k; ++r) s -= L[r * N + p] * out[r];
-                out[p] = s / L[p * N + p];
-            }
-        };
-        for (int q = 0; q < k; ++q) rb[q] = -c[ia[q]];
-        solve(rb, a);
-        double lam = 0.0;
-        if (closed) {
-            double sumcF = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
-            for (int q = 0; q < k; ++q) {
-                double s = 0.0;
-                for (int f = 0; f < N; ++f)
-                    if (!((A >> f) & 1u)) s += sC[ia[q] * N + f];
-                rb[q] = s;
-            }
-            solve(rb, b);
-            for (int f = 0; f < N; ++f) {
-                if ((A >> f) & 1u) continue;
-                sumcF += c[f];
-                for (int q = 0; q < k; ++q) {
-                    t1 += sC[f * N + ia[q]] * a[q];
-                    t3 += sC[f * N + ia[q]] * b[q];
-                }
-                for (int f2 = 0; f2 < N; ++f2)
-                    if (!((A >> f2) & 1u)) t2 += sC[f * N + f2];
-            }
-            lam = (Nhat - sumcF - t1) / (t2 - t3);
-            for (int q = 0; q < k; ++q) a[q] -= lam * b[q];
-        }
-        for (int q = 0; q < k; ++q)
-            if (a[q] - lam < -1e-9 * scale) failed = true;  // KKT: bound multipliers must be >= 0
-        for (int f = 0; f < N; ++f) {
-            if ((A >> f) & 1u) {
-                x[f] = 0.0;  // clamped components are exactly 0 (R3)
-                continue;
-            }
-            double s = c[f];
-            for (int q = 0; q < k; ++q) s += sC[f * N + ia[q]] * a[q];
+        qa_qp_eqp<N>(sC, c, closed, Nhat, A, x, r);
+        if (!general)
+            for (int i = 0; i < N; ++i)
+                if (r[i] < -1e-9 * scale) failed = true;  // KKT: bound multipliers must be >= 0
+    }
+    if (!general || failed || A == 0) return rounds;
+    // phase 2
+    const double tol = 1e-13 * scale;
+    double xe[N];
+    for (int it = 0; it < 50 * N + 50; ++it) {
+        if (A != 0) {
+            qa_qp_eqp<N>(sC, c, closed, Nhat, A, xe, r);  // |A| = N only for an open array (x = 0, r = -M c)
+        } else {  // every bound released: the face minimiser is the analytic minimum of S2
+            double lam = 0.0;
             if (closed) {
-                double rowF = 0.0;
-                for (int f2 = 0; f2 < N; ++f2)
-                    if (!((A >> f2) & 1u)) rowF += sC[f * N + f2];
-                s += lam * rowF;
-                if (k == N - 1) s = Nhat;  // R3: a single free dot carries the whole charge, exactly
+                double sc = 0.0, sCC = 0.0;
+                for (int i = 0; i < N; ++i) {
+                    sc += c[i];
+                    for (int j = 0; j < N; ++j) sCC += sC[i * N + j];
+                }
+                lam = (Nhat - sc) / sCC;
             }
-            x[f] = s;
+            for (int i = 0; i < N; ++i) {
+                double row = 0.0;
+                for (int j = 0; j < N; ++j) row += sC[i * N + j];
+                xe[i] = c[i] + lam * row;
+                r[i] = 0.0;
+            }
+        }
+        double pmax = 0.0;
+        for (int i = 0; i < N; ++i) pmax = fmax(pmax, fabs(xe[i] - x[i]));
+        ++rounds;
+        if (pmax <= tol) {
+            for (int i = 0; i < N; ++i) x[i] = xe[i];
+            int worst = -1;
+            double rmin = -1e-12 * scale;
+            for (int i = 0; i < N; ++i)
+                if (((A >> i) & 1u) && r[i] < rmin) {
+                    rmin = r[i];
+                    worst = i;
+                }
+            if (worst < 0) return rounds;  // KKT point
+            A &= ~(1u << worst);
+            continue;
+        }
+        double alpha = 1.0;
+        int block = -1;
+        for (int i = 0; i < N; ++i) {
+            if ((A >> i) & 1u) continue;
+            const double p = xe[i] - x[i];
+            if (p < 0.0) {
+                const double al = x[i] / (-p);
+                if (al < alpha) {
+                    alpha = al;
+                    block = i;
+                }
+            }
+        }
+        if (block < 0) {
+            for (int i = 0; i < N; ++i) x[i] = xe[i];
+        } else {
+            for (int i = 0; i < N; ++i)
+                if (!((A >> i) & 1u)) x[i] += alpha * (xe[i] - x[i]);
+            x[block] = 0.0;
+            A |= 1u << block;
         }
     }
+    failed = true;
     return rounds;
 }
 
@@ -196,7 +278,7 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
     // S3
     int rounds = 0;
     bool failed = false;
-    if (neg) rounds = qa_qp_clamp<N>(sC, nc, closed, (double)args.N_hat, x, failed);
+    if (neg) rounds = qa_qp_clamp<N>(sC, nc, closed, (double)args.N_hat, args.general_qp != 0, x, failed);
     // S4
     int32_t base[N], cnt[N];
     int doublings = 0;

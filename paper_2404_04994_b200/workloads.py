@@ -219,6 +219,23 @@ def random_open(n: int, g: int, P: int, seed: int, lo: float = -0.6, hi: float =
     return Workload(f"random_open_n{n}_g{g}_s{seed}", C_dd, C_gd, np.ascontiguousarray(Vg), P, 1)
 
 
+def random_general(n: int, g: int, P: int, seed: int, lo: float = -0.8, hi: float = 3.2) -> Workload:
+    """Test array whose c_dd is symmetric positive definite but NOT a Maxwell matrix: mutual terms of both signs, so some
+    off-diagonals of c_dd are positive (legal input, PAPER.md L204 asks only for SPD); diagonally dominant by
+    construction.  Exercises the general active-set phase of the continuous QP."""
+    rng = np.random.default_rng(seed)
+    C_m = np.triu(rng.uniform(-0.15, 0.25, size=(n, n)), 1)
+    C_m[0, 1] = -0.12                        # at least one positive off-diagonal in c_dd
+    C_m = C_m + C_m.T
+    C_gd = rng.uniform(0.0, 0.15, size=(n, g))
+    for i in range(min(n, g)):
+        C_gd[i, i] = rng.uniform(0.8, 1.2)
+    C_dd = np.diag(1.0 + C_gd.sum(1) + np.abs(C_m).sum(1)) - C_m
+    target = rng.uniform(lo, hi, size=(P, n))
+    Vg = target @ np.linalg.pinv(C_gd).T
+    return Workload(f"random_general_n{n}_g{g}_s{seed}", C_dd, C_gd, np.ascontiguousarray(Vg), P, 1)
+
+
 def shard_range(P: int, rank: int, world: int):
     """Contiguous pixel range [p0, p1) of rank `rank` of `world` (pixels are independent: SURVEY.md section 8(e))."""
     base, rem = divmod(P, world)

@@ -167,6 +167,24 @@ def test_all_sizes_closed_and_thresholded(api, n):
         check(api, w, algorithm="brute", n_max=3)
 
 
+# ---- c_dd with positive off-diagonals (SPD, not Maxwell): general active-set phase of the QP (reading R3) -------------
+@pytest.mark.parametrize("n", [2, 3, 5, 8, 11, 13, 16])
+def test_general_spd_matrices(api, n):
+    w = wl.random_general(n, n, 257 if n <= 11 else 41, seed=400 + n)
+    assert (w.C_dd - np.diag(np.diag(w.C_dd)) > 0).any()
+    rep, g, o = check(api, w, algorithm="default")
+    assert g["stats"]["n_qp_pixels"] > 0
+    if n >= 13:
+        assert g["plan"][0][1] == "qa_walk_kernel"      # the min-plus walk needs M >= 0 (Maxwell); exact walk here
+    if n <= 11:
+        check(api, w, algorithm="thresholded", t=0.3)
+        w.regime, w.N_hat = "closed", n
+        check(api, w, algorithm="default")
+        check(api, w, algorithm="thresholded", t=0.3)
+        if n <= 5:
+            check(api, w, algorithm="brute", n_max=3)
+
+
 # ---- edge cases -----------------------------------------------------------------------------------------------------
 def test_edge_cases(api):
     w = wl.config1(4, 4)
@@ -204,10 +222,9 @@ def test_edge_cases(api):
     with pytest.raises(api.QaError) as e:
         api.Model(np.eye(17), np.eye(17))
     assert e.value.status == 4
-    mp = api.Model(np.array([[1.0, 0.1], [0.1, 1.0]]), np.eye(2))
-    with pytest.raises(api.QaError) as e:
-        mp.ground_state(torch.from_numpy(w.Vg).cuda())
-    assert e.value.status == 8
+    mp = api.Model(np.array([[1.0, 0.1], [0.1, 1.0]]), np.eye(2))   # positive off-diagonal: legal (general QP phase)
+    r = mp.ground_state(torch.from_numpy(w.Vg).cuda())
+    assert (r["N"] >= 0).all()
     with pytest.raises(TypeError):
         m.ground_state(torch.from_numpy(w.Vg))          # no CPU path
 
