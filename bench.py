@@ -43,7 +43,6 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--arrays", type=int, default=256, help="config5: arrays of the dataset batch per GPU")
-    ap.add_argument("--streams", type=int, default=8, help="config5: CUDA streams the independent calls are spread over")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -285,9 +284,9 @@ def run_ours(args, rank, world, local_rank):
 def run_config5(args, rank, world, local_rank):
     """Secondary workload (BASELINE.json configs[4]): the dataset batch of independently seeded open 8-dot arrays, each a
     128x128 sweep, with the default algorithm and the thresholded one at t = 0.2 and 0.5.  One step = every array with
-    all three algorithms.  Arrays are independent calls of the single-model entry point, spread round-robin over a few
-    CUDA streams (each call is less than one wave of the GPU).  Reports pixels/s over the whole batch and the
-    agreement rate of thresholded vs default (fraction of pixels with identical N)."""
+    all three algorithms, through qa_ground_state_batch (semantically a loop over the single-model call, one launch of
+    the one-kernel path per algorithm).  Reports pixels/s over the whole batch and the agreement rate of thresholded vs
+    default (fraction of pixels with identical N)."""
     import torch
     import torch.distributed as dist
     from paper_2404_04994_b200 import api, workloads as wl
@@ -297,30 +296,19 @@ def run_config5(args, rank, world, local_rank):
     B = args.arrays
     wls = [wl.config5_array(j + B * rank) for j in range(B)]
     models = [api.Model(w.C_dd, w.C_gd) for w in wls]
-    Vgs = [torch.from_numpy(w.Vg).to(dev) for w in wls]
+    batch = api.Batch(models)                                    # qa_batch_create: one launch per algorithm
+    Vg = torch.from_numpy(np.stack([w.Vg for w in wls])).to(dev)  # [B, P, g]
     algs = (("default", dict(algorithm="default")), ("t0.2", dict(algorithm="thresholded", t=0.2)),
             ("t0.5", dict(algorithm="thresholded", t=0.5)))
-    outs = {a: [{"N": torch.empty((w.P, w.n_dot), dtype=torch.int32, device=dev),
-                 "E": torch.empty(w.P, dtype=torch.float64, device=dev)} for w in wls] for a, _ in algs}
-    # one model object per (array, algorithm): a model owns its workspace, and the three calls of an array may overlap
-    mods = {a: ([api.Model(w.C_dd, w.C_gd) for w in wls] if a != "default" else models) for a, _ in algs}
-    streams = [torch.cuda.Stream(dev) for _ in range(args.streams)]
-    px_step = sum(w.P for w in wls) * len(algs)
+    P, n = wls[0].P, wls[0].n_dot
+    outs = {a: {"N": torch.empty((B, P, n), dtype=torch.int32, device=dev),
+                "E": torch.empty((B, P), dtype=torch.float64, device=dev)} for a, _ in algs}
+    px_step = B * P * len(algs)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def step():
-        cur = torch.cuda.current_stream(dev)
-        for s_ in streams:
-            s_.wait_stream(cur)
-        k = 0
         for a, kw in algs:
-            for j in range(B):
-                s_ = streams[k % len(streams)]
-                k += 1
-                with torch.cuda.stream(s_):
-                    mods[a][j].ground_state(Vgs[j], out=outs[a][j], **kw)
-        for s_ in streams:
-            cur.wait_stream(s_)
+            batch.ground_state(Vg, out=outs[a], **kw)
 
     def barrier():
         if world > 1:
@@ -330,7 +318,7 @@ def run_config5(args, rank, world, local_rank):
     for _ in range(max(3, args.warmup)):
         flush.fill_(1)
         step()
-    launches_per_step = api.last_launch_plan()[1] * B * len(algs)
+    launches_per_step = api.last_launch_plan()[1] * len(algs)
     sampler = ClockSampler(local_rank)
     sampler.start()
     barrier()
@@ -353,8 +341,8 @@ def run_config5(args, rank, world, local_rank):
         return
     agree = {}
     for a in ("t0.2", "t0.5"):
-        same = sum(int((outs[a][j]["N"] == outs["default"][j]["N"]).all(dim=1).sum()) for j in range(B))
-        agree[a] = same / (px_step / len(algs))
+        same = int((outs[a]["N"] == outs["default"]["N"]).all(dim=2).sum())
+        agree[a] = same / (B * P)
     n, g = wls[0].n_dot, wls[0].n_gate
     bytes_px = 8 * g + 4 * n + 8                       # V_g in, N and E out
     hbm = None
@@ -369,11 +357,12 @@ def run_config5(args, rank, world, local_rank):
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[4]: {B} open 8-dot arrays (seeds 1000+j), 128x128 each, "
-                                   "default + thresholded t=0.2 + t=0.5", "arrays_per_gpu": B, "streams": len(streams),
+                                   "default + thresholded t=0.2 + t=0.5", "arrays_per_gpu": B,
+                       "api": "qa_ground_state_batch: one launch per algorithm over all arrays",
                        "pixels_per_step_per_gpu": px_step, "l2": "flushed (256 MiB write) between timed steps",
                        "parallelism": f"array-range x{world}"},
             "agreement_with_default": agree,
-            "roofline": {"bound": "hbm", "kernel": "whole step (prologue + walk/enumerate + finalize per call)",
+            "roofline": {"bound": "hbm", "kernel": "qa_fused_small_kernel (whole step: 3 launches)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                          "bytes_per_pixel": bytes_px,
                          "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm else "fallback 6516 GB/s (SURVEY.md)"},

@@ -133,6 +133,24 @@ QA_API qa_status qa_ground_state_host(const qa_model *model, const double *h_Vg,
                                qa_algorithm alg, double t, int n_max, int32_t *h_N, double *h_E, double *h_xcont,
                                double *h_Vsensor, qa_stats *h_stats);
 
+/* ---- dataset batch (BASELINE.json configs[4]) ------------------------------------------------------------------------ */
+
+/* A list of models that share n_dot (<= 8) and n_gate, have no sensor dots and live on the same device.  A batch call
+ * is semantically a loop over the single-model call -- array b reads V_g[b] and writes N[b], E[b] -- but runs as ONE
+ * launch of the one-kernel path (every step S1-S7 in registers, one thread per pixel).  The models must outlive the batch.
+ * models: host array of n_models handles.  Errors: QA_ERR_UNSUPPORTED_SIZE (n_dot > 8 or sensor dots),
+ * QA_ERR_INVALID_ARG (mixed shapes or devices, NULL). */
+typedef struct qa_batch qa_batch;
+QA_API qa_status qa_batch_create(const qa_model *const *models, int n_models, qa_batch **out);
+QA_API qa_status qa_batch_destroy(qa_batch *batch);
+QA_API int qa_batch_size(const qa_batch *batch);
+/* d_Vg device [n_models*P*n_gate], d_N device [n_models*P*n_dot] int32, d_E device [n_models*P], d_xcont device
+ * [n_models*P*n_dot] or NULL, d_stats device or NULL (summed over the batch).  closed = 0/1 (N_hat read when closed).
+ * Asynchronous on cuda_stream; needs no workspace.  Argument errors as for the single-model calls. */
+QA_API qa_status qa_ground_state_batch(const qa_batch *batch, const double *d_Vg, int64_t P, int closed, int N_hat,
+                                       qa_algorithm alg, double t, int n_max, int32_t *d_N, double *d_E, double *d_xcont,
+                                       qa_stats *d_stats, void *cuda_stream);
+
 /* ---- measurement aids -------------------------------------------------------------------------------------------- */
 
 /* Sustained FP64 issue rate of the current device: independent DFMA chains on every SM for about `seconds`.
@@ -146,9 +164,10 @@ QA_API qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s,
 QA_API qa_status qa_set_kernel_timing(int enable);
 QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernels);
 
-/* Which kernel scores the 2^n candidates of the open default algorithm for n_dot >= 13 (process-wide; cross-check aid,
- * the results are identical): 0 = the exact-compare Gray walk used for n_dot <= 12, 1 (default) = the min-plus walk with
- * its finish kernel.  Returns QA_ERR_INVALID_ARG for any other value. */
+/* Kernel selection (process-wide; cross-check aid, the results are identical): 0 = the three-kernel path for every n_dot
+ * (prologue, exact-compare Gray walk or enumeration, finalize), 1 (default) = the min-plus walk with its finish kernel for
+ * the open default search of n_dot >= 13 and the one-kernel path for n_dot <= 8.  Returns
+ * QA_ERR_INVALID_ARG for any other value. */
 QA_API qa_status qa_set_walk_variant(int variant);
 
 /* Names of the kernels the last ground-state call on this host thread enqueued (comma separated; static storage). */

@@ -23,7 +23,8 @@ STATUS_NAMES = ["QA_OK", "QA_ERR_INVALID_ARG", "QA_ERR_NOT_SYMMETRIC", "QA_ERR_N
 EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "qa_model_n_dot", "qa_model_n_gate",
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
            "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
-           "qa_get_kernel_timings", "qa_set_walk_variant", "qa_last_launch_plan",
+           "qa_get_kernel_timings", "qa_set_walk_variant", "qa_batch_create", "qa_batch_destroy", "qa_batch_size",
+           "qa_ground_state_batch", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
 
 
@@ -71,6 +72,10 @@ def lib() -> C.CDLL:
                                              vp, C.c_size_t, vp]
         l.qa_ground_state_host.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, vp, vp, vp,
                                            vp, vp]
+        l.qa_batch_create.argtypes = [vp, C.c_int, C.POINTER(vp)]
+        l.qa_batch_destroy.argtypes = [vp]
+        l.qa_batch_size.argtypes = [vp]
+        l.qa_ground_state_batch.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp, vp, vp]
         l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
         l.qa_set_kernel_timing.argtypes = [C.c_int]
         l.qa_set_walk_variant.argtypes = [C.c_int]
@@ -214,6 +219,56 @@ class Model:
             res["Vsensor"] = Vs
         if st is not None:
             res["stats"] = st.as_dict()
+        return res
+
+
+class Batch:
+    """qa_batch_create over a list of Model objects with the same n_dot (<= 8) and n_gate: one launch for the whole list."""
+
+    def __init__(self, models):
+        self.models = list(models)          # keep them alive
+        arr = (C.c_void_p * len(self.models))(*[m._h.value for m in self.models])
+        self._h = C.c_void_p()
+        _check(lib().qa_batch_create(arr, len(self.models), C.byref(self._h)), "qa_batch_create")
+        self.n_dot, self.n_gate = self.models[0].n_dot, self.models[0].n_gate
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().qa_batch_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __len__(self):
+        return int(lib().qa_batch_size(self._h))
+
+    def ground_state(self, Vg: torch.Tensor, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0,
+                     want_xcont=False, want_stats=False, out=None, stream=None):
+        """qa_ground_state_batch on a CUDA tensor Vg[B, P, n_gate] (float64).  Returns dict(N[B,P,n], E[B,P], ...)."""
+        if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
+            raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        B = len(self)
+        Vg = Vg.contiguous().view(B, -1, self.n_gate)
+        P, dev = Vg.shape[1], Vg.device
+        out = out or {}
+        N = out.get("N") if out.get("N") is not None else torch.empty((B, P, self.n_dot), dtype=torch.int32, device=dev)
+        E = out.get("E") if out.get("E") is not None else torch.empty((B, P), dtype=torch.float64, device=dev)
+        xc = torch.empty((B, P, self.n_dot), dtype=torch.float64, device=dev) if want_xcont else None
+        st = torch.zeros(8, dtype=torch.int64, device=dev) if want_stats else None
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        alg = ALG[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        _check(lib().qa_ground_state_batch(self._h, _ptr(Vg), P, int(regime == "closed"), int(N_hat), alg, float(t),
+                                           int(n_max), _ptr(N), _ptr(E), _ptr(xc), _ptr(st), C.c_void_p(s.cuda_stream)),
+               "qa_ground_state_batch")
+        res = {"N": N, "E": E}
+        if xc is not None:
+            res["xcont"] = xc
+        if st is not None:
+            res["stats"] = st
         return res
 
 

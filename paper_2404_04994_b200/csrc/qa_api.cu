@@ -10,6 +10,12 @@
 
 #include "qa_internal.cuh"
 
+struct qa_batch {
+    int n_models, n, g, general;
+    int device;
+    const QaDevModel **dev_list;  // device array of the models' device pointers
+};
+
 struct qa_model {
     int nf, g, ns;          // full model
     int device;
@@ -22,6 +28,7 @@ struct qa_model {
     int sens[QA_MAXN];
     QaDevModel host;        // mirror of the device constants
     QaDevModel *dev;        // device copy
+    const QaDevModel **dev_self;  // device array of one pointer (= dev): the model list of a single-model fused launch
     QaWalkTable walk;       // pair table of the low bits of the search model
     // qa_ground_state_host: a private stream and a grow-only device staging buffer, reused from call to call (creating
     // a stream and going through the allocator cost more than the search itself on a 100x100 diagram)
@@ -166,7 +173,8 @@ qa_status rebuild(qa_model *m)
 }
 
 // qa_set_walk_variant (cross-check aid): which kernel scores the open/default candidates of arrays with n >= 13.
-// 0 = exact-compare Gray walk (the n <= 12 kernel), 1 (default) = min-plus walk + finish kernel.  Initial value from the
+// 0 = the three-kernel path everywhere (prologue, exact-compare Gray walk or enumeration, finalize), 1 (default) = the
+// min-plus walk + finish kernel for n >= 13 and the one-kernel path for n <= 8.  Initial value from the
 // environment variable QA_WALK_VARIANT.
 int g_walk_variant = -1;
 int walk_variant()
@@ -238,6 +246,15 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1};
     g_n_marks = 0;
     timing_mark(stream);
+    // small arrays with small candidate sets: the whole path in one kernel, one thread per pixel (no workspace traffic)
+    {
+        const double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n) : std::pow(2.0, (double)n);
+        if (n <= QA_FUSED_MAXN && m->ns == 0 && expect <= 256.0 && walk_variant() != 0) {
+            QA_CUDA(qa_launch_fused_small(m->dev_self, 1, n, d_Vg, P, a, d_N, d_E, d_xcont, d_stats, stream));
+            timing_mark(stream);
+            return QA_OK;
+        }
+    }
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
     timing_mark(stream);
     // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd
@@ -314,13 +331,18 @@ qa_status qa_model_create(const double *C_dd, const double *C_gd, int n_dot, int
     cudaError_t e = cudaGetDevice(&m->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, m->device);
     if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&m->dev), sizeof(QaDevModel));
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&m->dev_self), sizeof(QaDevModel *));
+    if (e == cudaSuccess) e = cudaMemcpy(m->dev_self, &m->dev, sizeof(QaDevModel *), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
+        if (m->dev) cudaFree(m->dev);
+        if (m->dev_self) cudaFree(m->dev_self);
         delete m;
         return cuda_fail(e, "qa_model_create");
     }
     qa_status s = rebuild(m);
     if (s != QA_OK) {
         cudaFree(m->dev);
+        cudaFree(m->dev_self);
         delete m;
         return s;
     }
@@ -353,6 +375,7 @@ qa_status qa_model_destroy(qa_model *m)
 {
     if (!m) return QA_OK;
     cudaError_t e = cudaFree(m->dev);
+    if (m->dev_self) cudaFree(m->dev_self);
     if (m->host_buf) cudaFree(m->host_buf);
     if (m->host_stream) cudaStreamDestroy(m->host_stream);
     delete m;
@@ -445,6 +468,76 @@ qa_status qa_ground_state_host(const qa_model *mc, const double *h_Vg, int64_t P
     if (e2 != cudaSuccess) return cuda_fail(e2, "qa_ground_state_host sync");
     return QA_OK;
 }
+
+qa_status qa_batch_create(const qa_model *const *models, int n_models, qa_batch **out)
+{
+    if (out) *out = nullptr;
+    if (!models || !out || n_models < 1 || n_models > 65535) return QA_ERR_INVALID_ARG;
+    for (int b = 0; b < n_models; ++b) {
+        if (!models[b]) return QA_ERR_INVALID_ARG;
+        if (models[b]->ns != 0 || models[b]->host.n > QA_FUSED_MAXN) return QA_ERR_UNSUPPORTED_SIZE;
+        if (models[b]->host.n != models[0]->host.n || models[b]->g != models[0]->g ||
+            models[b]->device != models[0]->device)
+            return QA_ERR_INVALID_ARG;
+    }
+    qa_batch *bt = new (std::nothrow) qa_batch();
+    if (!bt) return QA_ERR_INVALID_ARG;
+    bt->n_models = n_models;
+    bt->n = models[0]->host.n;
+    bt->g = models[0]->g;
+    bt->device = models[0]->device;
+    const QaDevModel **list = new (std::nothrow) const QaDevModel *[n_models];
+    if (!list) {
+        delete bt;
+        return QA_ERR_INVALID_ARG;
+    }
+    for (int b = 0; b < n_models; ++b) {
+        list[b] = models[b]->dev;
+        if (!models[b]->is_z) bt->general = 1;
+    }
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&bt->dev_list), sizeof(QaDevModel *) * n_models);
+    if (e == cudaSuccess) e = cudaMemcpy(bt->dev_list, list, sizeof(QaDevModel *) * n_models, cudaMemcpyHostToDevice);
+    delete[] list;
+    if (e != cudaSuccess) {
+        if (bt->dev_list) cudaFree(bt->dev_list);
+        delete bt;
+        return cuda_fail(e, "qa_batch_create");
+    }
+    *out = bt;
+    return QA_OK;
+}
+
+qa_status qa_batch_destroy(qa_batch *bt)
+{
+    if (!bt) return QA_OK;
+    cudaError_t e = cudaFree(bt->dev_list);
+    delete bt;
+    return e == cudaSuccess ? QA_OK : cuda_fail(e, "qa_batch_destroy");
+}
+
+qa_status qa_ground_state_batch(const qa_batch *bt, const double *d_Vg, int64_t P, int closed, int N_hat, qa_algorithm alg,
+                                double t, int n_max, int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats,
+                                void *cuda_stream)
+{
+    qa_plan_reset();
+    if (!bt || P < 0 || (P > 0 && (!d_Vg || !d_N || !d_E))) return QA_ERR_INVALID_ARG;
+    if (alg != QA_ALG_DEFAULT && alg != QA_ALG_THRESHOLDED && alg != QA_ALG_BRUTE_FORCE) return QA_ERR_INVALID_ARG;
+    if (alg == QA_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return QA_ERR_INVALID_ARG;
+    if (alg == QA_ALG_BRUTE_FORCE && n_max < 0) return QA_ERR_INVALID_ARG;
+    if (closed && N_hat < 0) return QA_ERR_INFEASIBLE;
+    if (alg == QA_ALG_BRUTE_FORCE) {
+        if (std::pow((double)n_max + 1.0, (double)bt->n) >= 4.611686018427388e18) return QA_ERR_OVERFLOW;
+        if (closed && (int64_t)bt->n * n_max < N_hat) return QA_ERR_INFEASIBLE;
+    }
+    if (P == 0) return QA_OK;
+    if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, bt->general};
+    QA_CUDA(qa_launch_fused_small(bt->dev_list, bt->n_models, bt->n, d_Vg, P, a, d_N, d_E, d_xcont, d_stats,
+                                  static_cast<cudaStream_t>(cuda_stream)));
+    return QA_OK;
+}
+
+int qa_batch_size(const qa_batch *bt) { return bt ? bt->n_models : 0; }
 
 qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *cuda_stream)
 {

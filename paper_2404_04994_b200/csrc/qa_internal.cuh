@@ -9,6 +9,7 @@
 constexpr int QA_MAXN = 16;  // dots
 constexpr int QA_MAXG = 64;  // gates
 constexpr int QA_WALK_NL = 8;  // low bits walked per thread by the static Gray walk (2^8 candidates per thread)
+constexpr int QA_FUSED_MAXN = 8; // largest n of the one-kernel path (qa_kernels_fused.cu)
 constexpr int QA_PAIR_NL = 10; // low bits covered by the model's pair-energy table QL (min-plus walk: NL <= 10)
 
 // Pixel-independent model constants in device global memory (one per qa_model).
@@ -82,6 +83,9 @@ cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &
                            int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
                                    double *d_E, int sm_count, cudaStream_t stream);
+cudaError_t qa_launch_fused_small(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
+                                  QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats,
+                                  cudaStream_t stream);
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
                                double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int iters, cudaStream_t stream);

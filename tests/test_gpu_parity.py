@@ -58,7 +58,7 @@ def check(api, w, **kw):
 def test_config1_open_double_dot_default_and_brute(api):
     w = wl.config1(100, 100)
     rep, g, o = check(api, w, algorithm="default")
-    assert "qa_walk_kernel" in g["plan"][0]
+    assert g["plan"][0] == ["qa_fused_small_kernel"]
     assert st_zero_qp(g)
     check(api, w, algorithm="brute", n_max=5)
 
@@ -150,11 +150,29 @@ def test_config5_open_grid8_default_and_thresholded(api):
 @pytest.mark.parametrize("n", list(range(1, 17)))
 def test_all_sizes_default_open(api, n):
     w = wl.random_open(n, n + (n % 3), 301 if n <= 10 else (67 if n <= 13 else 37), seed=50 + n)
-    check(api, w, algorithm="default")
+    rep, g, o = check(api, w, algorithm="default")
+    if n <= 8:   # the one-kernel path above; the three-kernel path (static Gray walk) below
+        assert g["plan"][0] == ["qa_fused_small_kernel"]
+        try:
+            api.set_walk_variant(0)
+            rep, g0, o = check(api, w, algorithm="default")
+            assert g0["plan"][0] == ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"]
+            assert np.array_equal(g["N"], g0["N"])
+        finally:
+            api.set_walk_variant(1)
 
 
 @pytest.mark.parametrize("n", [1, 2, 3, 6, 9, 11])
-def test_all_sizes_closed_and_thresholded(api, n):
+@pytest.mark.parametrize("variant", [1, 0])
+def test_all_sizes_closed_and_thresholded(api, n, variant):
+    api.set_walk_variant(variant)
+    try:
+        _closed_and_thresholded(api, n)
+    finally:
+        api.set_walk_variant(1)
+
+
+def _closed_and_thresholded(api, n):
     w = wl.random_open(n, n, 203, seed=80 + n, lo=-0.4, hi=2.5)
     w.regime, w.N_hat = "closed", max(1, n)
     check(api, w, algorithm="default")
@@ -183,6 +201,38 @@ def test_general_spd_matrices(api, n):
         check(api, w, algorithm="thresholded", t=0.3)
         if n <= 5:
             check(api, w, algorithm="brute", n_max=3)
+
+
+# ---- dataset batch: one launch over several models == a loop over the single-model call ------------------------------
+def test_batch_equals_loop_and_oracle(api):
+    wls = [wl.config5_array(j, 40, 33) for j in range(5)]
+    models = [api.Model(w.C_dd, w.C_gd) for w in wls]
+    batch = api.Batch(models)
+    assert len(batch) == 5
+    Vg = torch.from_numpy(np.stack([w.Vg for w in wls])).cuda()
+    for kw in (dict(algorithm="default"), dict(algorithm="thresholded", t=0.2), dict(algorithm="thresholded", t=0.5),
+               dict(algorithm="default", regime="closed", N_hat=8)):
+        rb = batch.ground_state(Vg, want_xcont=True, want_stats=True, **kw)
+        torch.cuda.synchronize()
+        assert api.last_launch_plan()[0] == ["qa_fused_small_kernel"]
+        tot = 0
+        for j, (w, m) in enumerate(zip(wls, models)):
+            r1 = m.ground_state(Vg[j], **kw)
+            assert torch.equal(rb["N"][j], r1["N"]) and torch.equal(rb["E"][j], r1["E"])
+            om = oracle.Model(w.C_dd, w.C_gd)
+            okw = {k: v for k, v in kw.items() if k not in ("regime", "N_hat")}
+            o = om.ground_state(w.Vg, regime=kw.get("regime", "open"), N_hat=kw.get("N_hat", 0), **okw)
+            compare(rb["N"][j].cpu().numpy(), rb["E"][j].cpu().numpy(), o, om.EC, gpu_x=rb["xcont"][j].cpu().numpy())
+            tot += int(o["n_scored"].sum())
+        st = api.stats_dict(rb["stats"])
+        assert st["n_pixels"] == 5 * wls[0].P and st["n_candidates_scored"] == tot
+    with pytest.raises(api.QaError) as e:
+        api.Batch([models[0], api.Model(wl.config1(4, 4).C_dd, wl.config1(4, 4).C_gd)])
+    assert e.value.status == 1
+    w16 = wl.config4(2, 2)
+    with pytest.raises(api.QaError) as e:
+        api.Batch([api.Model(w16.C_dd, w16.C_gd)])
+    assert e.value.status == 4
 
 
 # ---- edge cases -----------------------------------------------------------------------------------------------------
