@@ -25,8 +25,9 @@ __host__ __device__ constexpr int fs_ctz(int k)
     return j;
 }
 
-template <int N>
-__global__ void __launch_bounds__(FS_THREADS) qa_fused_small_kernel(const QaDevModel *const *__restrict__ models,
+// GRAY: the open default set (compiled separately: the two scoring loops have very different register needs)
+template <int N, bool GRAY>
+__global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kernel(const QaDevModel *const *__restrict__ models,
                                                                     const double *__restrict__ Vg, int64_t P,
                                                                     QaCallArgs args, int32_t *__restrict__ outN,
                                                                     double *__restrict__ outE, double *__restrict__ xcont,
@@ -83,8 +84,8 @@ __global__ void __launch_bounds__(FS_THREADS) qa_fused_small_kernel(const QaDevM
     double best = INFINITY;
     uint64_t bidx = ~0ull;
     int64_t scored = 0;
-    const bool gray = args.alg == QA_ALG_DEFAULT && !closed;  // every cnt_i = 2: the static Gray walk of qa_kernels_walk.cu
-    if (gray) {
+    constexpr bool gray = GRAY;  // every cnt_i = 2: the static Gray walk of qa_kernels_walk.cu
+    if constexpr (GRAY) {
         // E(base + b) - E(base) = sum_i b_i h_i + QL[b], h_i = grad_i + 1/2 M_ii; low bit j <-> dot N-1-j; 3 FP64
         // instructions per candidate, every index static.  The winning pattern IS the mixed-radix index (cnt_i = 2).
         double hp[N];
@@ -189,7 +190,10 @@ cudaError_t launch_fused_n(const QaDevModel *const *d_models, int n_models, cons
                            int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats, cudaStream_t stream)
 {
     const dim3 grid((unsigned)((P + FS_THREADS - 1) / FS_THREADS), (unsigned)n_models);
-    qa_fused_small_kernel<N><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_stats);
+    if (args.alg == QA_ALG_DEFAULT && !args.closed)
+        qa_fused_small_kernel<N, true><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_stats);
+    else
+        qa_fused_small_kernel<N, false><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_stats);
     return cudaGetLastError();
 }
 
