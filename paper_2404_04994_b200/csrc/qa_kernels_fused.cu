@@ -110,7 +110,46 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
         bidx = idx;
         scored = (int64_t)total;
     }
-    const uint64_t len = (live && !gray) ? total : 0;
+    // Thresholded set of an open array: every dot has one or two values, i.e. base + a subset of the k free dots.  Walked in
+    // Gray order over the free dots (one rank-1 update per candidate instead of the odometer's ~two); the running key
+    // holds the digits with dot 0 most significant, so equal energies fall to the lexicographically smallest N (R6).
+    const bool subset = !GRAY && !closed && args.alg == QA_ALG_THRESHOLDED;
+    if (!GRAY && subset && live) {
+        unsigned flist = 0;  // 4-bit dot indices of the free dots, highest dot first
+        int k = 0;
+#pragma unroll
+        for (int i = N - 1; i >= 0; --i)
+            if (cnt[i] == 2) flist |= (unsigned)i << (4 * k++);
+        unsigned key = 0, bkey = 0;
+        best = E;
+        for (unsigned st = 1; st < (1u << k); ++st) {
+            const int i = (int)((flist >> (4 * (__ffs(st) - 1))) & 15u);
+            const unsigned bit = 1u << (N - 1 - i);
+            const double dl = (key & bit) ? -1.0 : 1.0;
+            double gi = 0.0;
+#pragma unroll
+            for (int j = 0; j < N; ++j)
+                if (j == i) gi = grad[j];
+            E += dl * (gi + 0.5 * dl * sM[i * N + i]);
+#pragma unroll
+            for (int j = 0; j < N; ++j) grad[j] = fma(dl, sM[j * N + i], grad[j]);
+            key ^= bit;
+            if (E < best || (E == best && key < bkey)) {
+                best = E;
+                bkey = key;
+            }
+        }
+        // key -> mixed-radix index of the shared decode below
+        uint64_t w = 1, idx = 0;
+#pragma unroll
+        for (int i = N - 1; i >= 0; --i) {
+            idx += (uint64_t)((bkey >> (N - 1 - i)) & 1u) * w;
+            w *= (uint64_t)cnt[i];
+        }
+        bidx = idx;
+        scored = (int64_t)total;
+    }
+    const uint64_t len = (live && !gray && !subset) ? total : 0;
     for (uint64_t it = 0; it < len; ++it) {
         if (!closed || sumN == args.N_hat) {
             ++scored;
