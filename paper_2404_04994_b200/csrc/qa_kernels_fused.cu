@@ -139,14 +139,7 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
                 bkey = key;
             }
         }
-        // key -> mixed-radix index of the shared decode below
-        uint64_t w = 1, idx = 0;
-#pragma unroll
-        for (int i = N - 1; i >= 0; --i) {
-            idx += (uint64_t)((bkey >> (N - 1 - i)) & 1u) * w;
-            w *= (uint64_t)cnt[i];
-        }
-        bidx = idx;
+        bidx = bkey;  // binary digits, dot 0 most significant (decoded without division below)
         scored = (int64_t)total;
     }
     const uint64_t len = (live && !gray && !subset) ? total : 0;
@@ -187,15 +180,21 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
     if (live) {
         const bool empty = bidx == ~0ull;
         int32_t Ns[N];
-        uint64_t idx = bidx;
+        if (gray || subset) {  // the winner's digits are the bits of bidx (64-bit division is ~100 instructions a digit)
 #pragma unroll
-        for (int i = N - 1; i >= 0; --i) {
-            const uint64_t c = (uint64_t)cnt[i];
-            const int32_t dgt = (int32_t)(idx % c);
-            idx /= c;
-            Ns[i] = empty ? -1 : base[i] + dgt;
-            d[i] = (double)Ns[i] - nc[i];
+            for (int i = 0; i < N; ++i) Ns[i] = base[i] + (int32_t)((bidx >> (N - 1 - i)) & 1ull);
+        } else {
+            uint64_t idx = bidx;
+#pragma unroll
+            for (int i = N - 1; i >= 0; --i) {
+                const uint64_t c = (uint64_t)cnt[i];
+                const int32_t dgt = (int32_t)(idx % c);
+                idx /= c;
+                Ns[i] = empty ? -1 : base[i] + dgt;
+            }
         }
+#pragma unroll
+        for (int i = 0; i < N; ++i) d[i] = (double)Ns[i] - nc[i];
         double Ed = 0.0;
 #pragma unroll
         for (int i = 0; i < N; ++i) {
