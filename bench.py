@@ -2,7 +2,7 @@
 """bench.py -- throughput of the ground-state charge search on the headline workload (BASELINE.json configs[3]:
 open 4x4 grid of 16 dots, default algorithm, 100x100 pixels, 2^16 candidates per pixel, fp64).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config5]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config5|small]
 
 One "step" = one pass of the whole hot path (prologue -> candidate walk -> finalize) over
 one 100x100 diagram.  Prints ONE JSON line (rank 0).  Multi-GPU: one process per GPU (torchrun), every rank runs its own
@@ -39,7 +39,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config4", "config5"])
+    ap.add_argument("--workload", default="config4", choices=["config4", "config5", "small"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--arrays", type=int, default=256, help="config5: arrays of the dataset batch per GPU")
@@ -370,6 +370,47 @@ def run_config5(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------------------------------
+def run_small(args, rank):
+    """BASELINE.json configs[0..2] (launch-latency-bound diagrams: 10^4 - 4*10^4 pixels, <= 7776 candidates per pixel):
+    device time of one diagram per (config, algorithm), CUDA events, L2 flushed between repetitions.  One JSON line."""
+    if rank != 0:
+        return
+    import torch
+    from paper_2404_04994_b200 import api, workloads as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    cases = [("config1 open double dot 100x100", wl.config1(100, 100), [dict(algorithm="default"), dict(algorithm="brute", n_max=5)]),
+             ("config2 closed 5-chain N=5 100x100", wl.config2(100, 100), [dict(algorithm="default"), dict(algorithm="brute", n_max=5)]),
+             ("config3 open 2x2 + sensor 200x200", wl.config3(200, 200), [dict(algorithm="default")])]
+    rows = []
+    for name, w, kws in cases:
+        m = api.Model(w.C_dd, w.C_gd, sensor_dots=w.sensor_dots)
+        Vg = torch.from_numpy(w.Vg).to(dev)
+        for kw in kws:
+            for _ in range(max(3, args.warmup)):
+                m.ground_state(Vg, regime=w.regime, N_hat=w.N_hat, **kw)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            for k in range(args.steps):
+                flush.fill_(k & 0xff)
+                ev[k][0].record()
+                r = m.ground_state(Vg, regime=w.regime, N_hat=w.N_hat, want_stats=(k == 0), **kw)
+                ev[k][1].record()
+                if k == 0:
+                    st = r["stats"]
+            torch.cuda.synchronize()
+            t = np.array([a.elapsed_time(b) for a, b in ev[1:]])
+            sd = api.stats_dict(st)
+            rows.append({"config": name, "algorithm": kw["algorithm"], "pixels": w.P, "ms_median": float(np.median(t)),
+                         "ms_min": float(t.min()), "pixels_per_s": w.P / (float(np.median(t)) * 1e-3),
+                         "candidates_enumerated": sd["n_candidates_enumerated"], "candidates_scored": sd["n_candidates_scored"],
+                         "qp_pixels": sd["n_qp_pixels"], "kernels": api.last_launch_plan()[0]})
+    print(json.dumps({"metric": "device time per diagram, BASELINE.json configs[0..2]", "unit": "ms", "n_gpus": 1,
+                      "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
+                      "l2": "flushed (256 MiB write) between repetitions", "rows": rows}), flush=True)
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0"))
@@ -387,7 +428,9 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl")
         dist.barrier()
-    if args.workload == "config5":
+    if args.workload == "small":
+        run_small(args, rank)
+    elif args.workload == "config5":
         run_config5(args, rank, world, local_rank)
     else:
         run_ours(args, rank, world, local_rank)
