@@ -35,6 +35,8 @@ def _lib(omp: bool = False):
         lib.qo_continuous_min.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         lib.qo_ground_state.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp,
                                         lp, lp, ip, ip, C.c_int]
+        lib.qo_thermal.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp,
+                                   lp, ip]
         lib.qo_sensor.argtypes = [vp, vp, ip, C.c_int, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip,
                                   dp, dp, dp, ip]
         _libs[key] = lib
@@ -140,6 +142,21 @@ class Model:
         if rc:
             raise ValueError(f"qo_ground_state: invalid argument ({rc})")
         return out
+
+
+def _thermal(self, Vg, kT, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0):
+    """Eq. (10): Boltzmann-weighted mean occupation over the candidate set.  Returns dict(Nmean[P,n], Emin[P], n_scored, flags)."""
+    Vg = np.ascontiguousarray(Vg, dtype=np.float64).reshape(-1, self.g)
+    P = Vg.shape[0]
+    out = dict(Nmean=np.empty((P, self.n)), Emin=np.empty(P), n_scored=np.empty(P, np.int64), flags=np.empty(P, np.int32))
+    rc = _lib().qo_thermal(self._buf, _dp(Vg), P, int(regime == "closed"), int(N_hat), ALG[algorithm], float(t), int(n_max),
+                           float(kT), _dp(out["Nmean"]), _dp(out["Emin"]), _lp(out["n_scored"]), _ip(out["flags"]))
+    if rc:
+        raise ValueError(f"qo_thermal: invalid argument ({rc})")
+    return out
+
+
+Model.thermal = _thermal
 
 
 def sensor_ground_state(C_dd, C_gd, sensor_dots, Vg, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0):

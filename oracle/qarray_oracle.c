@@ -19,8 +19,10 @@
  *      code, no incremental update, no blocking
  *   5. argmin (Eq. (5)), ties -> lexicographically smallest N (reading R6); also the second-best energy
  *   6. charge-sensor dots (L149, Eq. (3); reading R8)
+ *   7. thermal broadening: the soft arg min of Eq. (10) L157 over the same candidate set (qo_thermal; reading R13)
  *
- * Pins (tests/test_oracle_*.py): P0..P12 of DESIGN.md.  Functions with no pin independent of the oracle itself:
+ * Pins (tests/test_oracle_*.py): P0..P13 of DESIGN.md (P13: Eq. (10) -- Fermi function of a single dot, kT -> 0 and
+ * kT -> infinity limits, Eq. (4)-energy numpy sums on tiny arrays, sum <N> = N_hat).  Functions with no pin independent of the oracle itself:
  *   - qo_sensor's potential values on random arrays                           : "parity unpinned" beyond the
  *     single-sensor closed form tested in tests/test_oracle_pins.py (rounding of s, V_s = [M (N - N_c)]_s)
  *   - thresholded-vs-default agreement RATE on config 5                       : parity unpinned (statistic only)
@@ -457,6 +459,106 @@ int qo_pixel(const qo_model *m, const double *Vg, int closed, int N_hat, int alg
     if (n_enum) *n_enum = b.n_enum;
     if (n_doublings) *n_doublings = doublings;
     return flags;
+}
+
+/* ------------------------------------------------------------------------------------------------------------------ */
+/* Thermal broadening (section IV.B, Eq. (10)): the arg min of Eq. (5) is replaced by the Boltzmann-weighted   */
+/* mean over the SAME candidate set (steps 1-3 above; closed: only sum N = N_hat, L159):                                 */
+/*     <N> = sum_N N exp(-F(N)/kT) / sum_N exp(-F(N)/kT)                                                                 */
+/* kT > 0 is k_B T in the energy units of E (|e| = 1, R11).  Eq. (4) and the completed square E differ by a per-pixel    */
+/* constant, which cancels in the ratio; the weights are formed as exp(-(E - E_min)/kT) (E_min = smallest energy of the  */
+/* set) so that the largest weight is exactly 1.  Two plain passes in lexicographic order, energy from the definition.  */
+/* Nmean[n] (all -1 if the set is empty), *Emin.  returns flags.                                                         */
+int qo_pixel_thermal(const qo_model *m, const double *Vg, int closed, int N_hat, int alg, double t, int n_max, double kT,
+                     double *Nmean, double *Emin, int64_t *n_scored)
+{
+    int n = m->n;
+    int32_t Nbest[QO_MAXN];
+    double E, E2, x[QO_MAXN];
+    int64_t ns = 0, ne = 0;
+    int32_t dbl = 0;
+    /* steps 1-3 and E_min: exactly the ground-state search (its candidate ranges are recomputed below the same way) */
+    int flags = qo_pixel(m, Vg, closed, N_hat, alg, t, n_max, Nbest, &E, &E2, x, &ns, &ne, &dbl);
+    if (n_scored) *n_scored = ns;
+    *Emin = E;
+    if (ns == 0) {
+        for (int i = 0; i < n; i++) Nmean[i] = -1.0;
+        return flags;
+    }
+    double Nc[QO_MAXN];
+    int32_t base[QO_MAXN], cnt[QO_MAXN];
+    qo_nc(m, Vg, Nc);
+    if (alg == QO_ALG_BRUTE) {
+        for (int i = 0; i < n; i++) {
+            base[i] = 0;
+            cnt[i] = n_max + 1;
+        }
+    } else {
+        double tt = (alg == QO_ALG_THRESHOLDED) ? t : 1.0;
+        ranges_floor_ceil(n, x, tt, alg == QO_ALG_THRESHOLDED, base, cnt);
+        if (closed) {
+            while (alg == QO_ALG_THRESHOLDED && !closed_nonempty(n, base, cnt, N_hat) && tt < 1.0) {
+                tt = (tt > 0.0) ? fmin(1.0, 2.0 * tt) : 1.0;
+                ranges_floor_ceil(n, x, tt, 1, base, cnt);
+            }
+            if (!closed_nonempty(n, base, cnt, N_hat)) {
+                for (int i = 0; i < n; i++) {
+                    double fl = floor(x[i]);
+                    int32_t lo = fl > 0.0 ? (int32_t)fl : 0;
+                    base[i] = lo > 0 ? lo - 1 : 0;
+                    cnt[i] = lo + 2 - base[i] + 1;
+                }
+            }
+        }
+    }
+    double Z = 0.0, S[QO_MAXN];
+    int32_t N[QO_MAXN];
+    for (int i = 0; i < n; i++) {
+        S[i] = 0.0;
+        N[i] = base[i];
+    }
+    for (;;) {
+        int ok = 1;
+        if (closed) {
+            int64_t s = 0;
+            for (int i = 0; i < n; i++) s += N[i];
+            ok = (s == N_hat);
+        }
+        if (ok) {
+            double w = exp(-(qo_energy(m, Nc, N) - E) / kT);
+            Z += w;
+            for (int i = 0; i < n; i++) S[i] += w * (double)N[i];
+        }
+        int i = n - 1;
+        while (i >= 0) {
+            if (N[i] < base[i] + cnt[i] - 1) {
+                N[i]++;
+                break;
+            }
+            N[i] = base[i];
+            i--;
+        }
+        if (i < 0) break;
+    }
+    for (int i = 0; i < n; i++) Nmean[i] = S[i] / Z;
+    return flags;
+}
+
+int qo_thermal(const qo_model *m, const double *Vg, int64_t P, int closed, int N_hat, int alg, double t, int n_max,
+               double kT, double *Nmean, double *Emin, int64_t *n_scored, int32_t *flags)
+{
+    if (!m || !Vg || !Nmean || !Emin || P < 0 || !(kT > 0.0)) return 1;
+    if (alg < 0 || alg > 2) return 1;
+    if (alg == QO_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return 1;
+    if (alg == QO_ALG_BRUTE && n_max < 0) return 1;
+    if (closed && N_hat < 0) return 1;
+    int n = m->n, g = m->g;
+    for (int64_t p = 0; p < P; p++) {
+        int f = qo_pixel_thermal(m, Vg + p * g, closed, N_hat, alg, t, n_max, kT, Nmean + p * n, Emin + p,
+                                 n_scored ? n_scored + p : 0);
+        if (flags) flags[p] = f;
+    }
+    return 0;
 }
 
 /* whole sweep: Vg[P][g] -> N[P][n], E[P], optional E2[P], xcont[P][n], n_scored[P], n_enum[P], flags[P], doublings[P].

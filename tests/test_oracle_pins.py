@@ -553,3 +553,75 @@ def test_openmp_variant_is_the_same_function():
     a = m.ground_state(w.Vg, regime="closed", N_hat=5)
     b = m.ground_state(w.Vg, regime="closed", N_hat=5, n_threads=4)
     assert np.array_equal(a["N"], b["N"]) and np.array_equal(a["E"], b["E"])
+
+
+# ---- P13: thermal broadening, Eq. (10) (L153-L159) -------------------------------------------------------------------
+def _softargmin_numpy(C_dd, C_gd, vg, cands, kT):
+    """Independent route: Eq. (4) free energy (NOT the completed square the oracle uses) and plain numpy sums."""
+    M = np.linalg.inv(C_dd)
+    q = np.asarray(cands, float)                                   # [K, n]
+    nc = C_gd @ vg
+    F = 0.5 * np.einsum("ki,ij,kj->k", q, M, q) - q @ (M @ nc)      # Eq. (4) L45 (positive-C_gd convention, R0b)
+    w = np.exp(-(F - F.min()) / kT)
+    return (w[:, None] * q).sum(0) / w.sum()
+
+
+def test_P13_single_dot_is_a_fermi_function():
+    """n = 1, default: candidates lo, lo+1 with E(N) = 1/2 M (N - N_c)^2, so <N> = lo + 1 / (1 + exp(dE / kT)),
+    dE = E(lo+1) - E(lo) = M (lo - N_c) + M / 2: a Fermi function centred on the half-integer."""
+    C = np.array([[1.7]])
+    m = oracle.Model(C, np.array([[0.9]]))
+    M = 1.0 / 1.7
+    vg = np.linspace(0.05, 4.0, 173)[:, None]
+    for kT in (0.004, 0.03, 0.4):
+        o = m.thermal(vg, kT)
+        nc = 0.9 * vg[:, 0]
+        lo = np.floor(nc)
+        dE = M * (lo - nc) + 0.5 * M
+        assert np.allclose(o["Nmean"][:, 0], lo + 1.0 / (1.0 + np.exp(dE / kT)), rtol=0, atol=1e-13)
+        assert np.allclose(o["Emin"], 0.5 * M * np.minimum(nc - lo, lo + 1 - nc) ** 2, atol=1e-15)
+
+
+@pytest.mark.parametrize("regime,N_hat", [("open", 0), ("closed", 3)])
+def test_P13_limits_and_independent_sum(regime, N_hat):
+    n = 4
+    C_dd, C_gd = chain(n, 21)
+    m = oracle.Model(C_dd, C_gd)
+    rng = np.random.default_rng(5)
+    Vg = rng.uniform(0.1, 2.2, size=(60, n)) @ np.linalg.inv(C_gd).T
+    g = m.ground_state(Vg, regime=regime, N_hat=N_hat)
+    EC = m.EC
+    # kT -> 0: the arg min of Eq. (5), wherever the runner-up is not within reach
+    cold = m.thermal(Vg, 1e-4 * EC, regime=regime, N_hat=N_hat)
+    clear = g["E2"] - g["E"] > 1e-2 * EC
+    assert clear.sum() > 40 and np.allclose(cold["Nmean"][clear], g["N"][clear], atol=1e-12)
+    assert np.array_equal(cold["Emin"], g["E"])
+    # kT -> infinity: the plain mean of the candidate set
+    hot = m.thermal(Vg, 1e12 * EC, regime=regime, N_hat=N_hat)
+    lo = np.maximum(np.floor(g["x"]), 0)
+    for p in range(len(Vg)):
+        cands = [lo[p] + np.array(b) for b in itertools.product((0, 1), repeat=n)]
+        if regime == "closed":
+            cands = [c for c in cands if c.sum() == N_hat]
+        assert np.allclose(hot["Nmean"][p], np.mean(cands, axis=0), atol=1e-9)
+        # in between: Eq. (10) written out with Eq. (4) energies (per-pixel constants cancel)
+        for kT in (0.02 * EC, 0.5 * EC):
+            o = m.thermal(Vg[p:p + 1], kT, regime=regime, N_hat=N_hat)
+            assert np.allclose(o["Nmean"][0], _softargmin_numpy(C_dd, C_gd, Vg[p], cands, kT), rtol=1e-10, atol=1e-12)
+    if regime == "closed":   # constraint (iii) survives the average
+        warm = m.thermal(Vg, 0.1 * EC, regime=regime, N_hat=N_hat)
+        assert np.allclose(warm["Nmean"].sum(1), N_hat, atol=1e-12)
+
+
+def test_P13_brute_force_box_and_bounds():
+    C_dd, C_gd = chain(3, 8)
+    m = oracle.Model(C_dd, C_gd)
+    rng = np.random.default_rng(2)
+    Vg = rng.uniform(0.0, 2.5, size=(25, 3)) @ np.linalg.inv(C_gd).T
+    o = m.thermal(Vg, 0.07 * m.EC, algorithm="brute", n_max=3)
+    box = [np.array(c, float) for c in itertools.product(range(4), repeat=3)]
+    for p in range(len(Vg)):
+        assert np.allclose(o["Nmean"][p], _softargmin_numpy(C_dd, C_gd, Vg[p], box, 0.07 * m.EC), rtol=1e-10, atol=1e-12)
+    assert (o["Nmean"] >= 0).all() and (o["Nmean"] <= 3).all()
+    with pytest.raises(ValueError):
+        m.thermal(Vg, 0.0)
