@@ -2,7 +2,7 @@
 """bench.py -- throughput of the ground-state charge search on the headline workload (BASELINE.json configs[3]:
 open 4x4 grid of 16 dots, default algorithm, 100x100 pixels, 2^16 candidates per pixel, fp64).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config5|small]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config5|small|thermal]
 
 One "step" = one pass of the whole hot path (prologue -> candidate walk -> finalize) over
 one 100x100 diagram.  Prints ONE JSON line (rank 0).  Multi-GPU: one process per GPU (torchrun), every rank runs its own
@@ -39,7 +39,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config4", "config5", "small"])
+    ap.add_argument("--workload", default="config4", choices=["config4", "config5", "small", "thermal"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--arrays", type=int, default=256, help="config5: arrays of the dataset batch per GPU")
@@ -411,6 +411,53 @@ def run_small(args, rank):
                       "l2": "flushed (256 MiB write) between repetitions", "rows": rows}), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------------------------------
+def run_thermal(args, rank):
+    """thermal broadening (Eq. (10)) on the config-4 diagram (16 dots, 100x100, default set: 2^16
+    Boltzmann weights per pixel), kT = 0.05 E_C.  Device time per diagram (CUDA events, L2 flushed) and the oracle on one
+    host core on a bounded sample.  One JSON line."""
+    if rank != 0:
+        return
+    import torch
+    import oracle
+    from paper_2404_04994_b200 import api, workloads as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    w = wl.config4(100, 100)
+    m = api.Model(w.C_dd, w.C_gd)
+    _, EC = m.inverse()
+    kT = 0.05 * EC
+    Vg = torch.from_numpy(w.Vg).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for _ in range(max(3, args.warmup)):
+        m.thermal(Vg, kT)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)
+        ev[k][0].record()
+        r = m.thermal(Vg, kT)
+        ev[k][1].record()
+    torch.cuda.synchronize()
+    t = np.array([a.elapsed_time(b) for a, b in ev])
+    kt = api.kernel_times(m, Vg, steps=5, flush=flush) if False else None
+    om = oracle.Model(w.C_dd, w.C_gd)
+    sel = np.sort(np.random.default_rng(0).choice(w.P, size=40, replace=False))
+    t0 = time.perf_counter()
+    o = om.thermal(w.Vg[sel], kT)
+    dt = time.perf_counter() - t0
+    err = float(np.abs(r["Nmean"].cpu().numpy()[sel] - o["Nmean"]).max())
+    ms = float(np.median(t))
+    print(json.dumps({"metric": "Boltzmann-weighted candidate configs/s (thermal broadening, 16 dots, default set, 100x100)",
+                      "value": w.P * 65536 / (ms * 1e-3), "unit": "candidates/s", "n_gpus": 1, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_min": float(t.min()), "higher_is_better": True,
+                      "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": "BASELINE.json configs[3] with Eq. (10), kT = 0.05 E_C", "kT": kT,
+                                 "l2": "flushed (256 MiB write) between timed steps"},
+                      "kernels_per_step": api.last_launch_plan()[0], "max_abs_err_vs_oracle_sample": err,
+                      "cpu_baseline": {"value": len(sel) * 65536 / dt, "unit": "candidates/s", "cores": 1, "kind": "oracle",
+                                       "sample": f"{len(sel)} of 10000 pixels (seeded random subset), {dt:.1f} s"}}), flush=True)
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0"))
@@ -428,7 +475,9 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl")
         dist.barrier()
-    if args.workload == "small":
+    if args.workload == "thermal":
+        run_thermal(args, rank)
+    elif args.workload == "small":
         run_small(args, rank)
     elif args.workload == "config5":
         run_config5(args, rank, world, local_rank)

@@ -133,6 +133,24 @@ QA_API qa_status qa_ground_state_host(const qa_model *model, const double *h_Vg,
                                qa_algorithm alg, double t, int n_max, int32_t *h_N, double *h_E, double *h_xcont,
                                double *h_Vsensor, qa_stats *h_stats);
 
+/* ---- thermal broadening (section IV.B, Eq. (10)) ------------------------------------------------------- */
+
+/* The arg min of Eq. (5) replaced by the soft arg min of Eq. (10): the Boltzmann-weighted mean of the charge states of the
+ * SAME candidate set the chosen algorithm enumerates (closed: only sum N = N_hat, L159),
+ *     <N> = sum_N N exp(-E(N)/kT) / sum_N exp(-E(N)/kT).
+ * kT > 0 (finite) is k_B T in the energy units of E (|e| = 1; reading R13); QA_ERR_INVALID_ARG otherwise.
+ *   d_Nmean  device [P*n_search] fp64   mean occupation of the searched dots (-1 where the candidate set is empty)
+ *   d_Emin   device [P] or NULL         smallest energy of the candidate set (= E(N*) of the ground-state search, evaluated
+ *                                       incrementally: not bit-identical to qa_ground_state's d_E)
+ * Other arguments, workspace, stream semantics and errors as qa_ground_state_open / _closed.  Sensor dots are not part of
+ * the average (the search model of qa_model_set_sensor_dots is used). */
+QA_API qa_status qa_thermal_open(const qa_model *model, const double *d_Vg, int64_t P, qa_algorithm alg, double t, int n_max,
+                                 double kT, double *d_Nmean, double *d_Emin, qa_stats *d_stats, void *d_workspace,
+                                 size_t workspace_bytes, void *cuda_stream);
+QA_API qa_status qa_thermal_closed(const qa_model *model, const double *d_Vg, int64_t P, int N_hat, qa_algorithm alg, double t,
+                                   int n_max, double kT, double *d_Nmean, double *d_Emin, qa_stats *d_stats,
+                                   void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* ---- dataset batch (BASELINE.json configs[4]) ------------------------------------------------------------------------ */
 
 /* A list of models that share n_dot (<= 8) and n_gate, have no sensor dots and live on the same device.  A batch call

@@ -24,7 +24,7 @@ EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "q
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
            "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
            "qa_get_kernel_timings", "qa_set_walk_variant", "qa_batch_create", "qa_batch_destroy", "qa_batch_size",
-           "qa_ground_state_batch", "qa_last_launch_plan",
+           "qa_ground_state_batch", "qa_thermal_open", "qa_thermal_closed", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
 
 
@@ -76,6 +76,9 @@ def lib() -> C.CDLL:
         l.qa_batch_destroy.argtypes = [vp]
         l.qa_batch_size.argtypes = [vp]
         l.qa_ground_state_batch.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp, vp, vp]
+        l.qa_thermal_open.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp, vp, vp, C.c_size_t, vp]
+        l.qa_thermal_closed.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp, vp, vp,
+                                        C.c_size_t, vp]
         l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
         l.qa_set_kernel_timing.argtypes = [C.c_int]
         l.qa_set_walk_variant.argtypes = [C.c_int]
@@ -188,6 +191,35 @@ class Model:
             res["xcont"] = xc
         if Vs is not None:
             res["Vsensor"] = Vs
+        if st is not None:
+            res["stats"] = st
+        return res
+
+    def thermal(self, Vg: torch.Tensor, kT: float, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0,
+                want_stats=False, stream=None):
+        """qa_thermal_open / qa_thermal_closed: Eq. (10) mean occupation on a CUDA tensor Vg[P, n_gate].  Returns
+        dict(Nmean[P, n_search] float64, Emin[P][, stats])."""
+        if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
+            raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        Vg = Vg.contiguous().view(-1, self.n_gate)
+        P, dev = Vg.shape[0], Vg.device
+        Nm = torch.empty((P, self.n_search), dtype=torch.float64, device=dev)
+        Em = torch.empty(P, dtype=torch.float64, device=dev)
+        st = torch.zeros(8, dtype=torch.int64, device=dev) if want_stats else None
+        ws = self._workspace(P, dev)
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        sp = C.c_void_p(s.cuda_stream)
+        alg = ALG[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        if regime == "open":
+            rc = lib().qa_thermal_open(self._h, _ptr(Vg), P, alg, float(t), int(n_max), float(kT), _ptr(Nm), _ptr(Em),
+                                       _ptr(st), _ptr(ws), ws.numel(), sp)
+        elif regime == "closed":
+            rc = lib().qa_thermal_closed(self._h, _ptr(Vg), P, int(N_hat), alg, float(t), int(n_max), float(kT), _ptr(Nm),
+                                         _ptr(Em), _ptr(st), _ptr(ws), ws.numel(), sp)
+        else:
+            raise ValueError("regime must be 'open' or 'closed'")
+        _check(rc, f"qa_thermal_{regime}")
+        res = {"Nmean": Nm, "Emin": Em}
         if st is not None:
             res["stats"] = st
         return res

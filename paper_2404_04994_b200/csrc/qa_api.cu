@@ -278,6 +278,43 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     return QA_OK;
 }
 
+// Thermal broadening (Eq. (10)): prologue (S1-S4) + qa_thermal_kernel.
+qa_status thermal(const qa_model *m, const double *d_Vg, int64_t P, int closed, int N_hat, qa_algorithm alg, double t,
+                  int n_max, double kT, double *d_Nmean, double *d_Emin, qa_stats *d_stats, void *d_ws, size_t ws_bytes,
+                  void *stream_v)
+{
+    qa_plan_reset();
+    if (!m || P < 0 || (P > 0 && (!d_Vg || !d_Nmean))) return QA_ERR_INVALID_ARG;
+    if (!(kT > 0.0) || !std::isfinite(kT)) return QA_ERR_INVALID_ARG;
+    if (alg != QA_ALG_DEFAULT && alg != QA_ALG_THRESHOLDED && alg != QA_ALG_BRUTE_FORCE) return QA_ERR_INVALID_ARG;
+    if (alg == QA_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return QA_ERR_INVALID_ARG;
+    if (alg == QA_ALG_BRUTE_FORCE && n_max < 0) return QA_ERR_INVALID_ARG;
+    const int n = m->host.n;
+    if (closed && N_hat < 0) return QA_ERR_INFEASIBLE;
+    if (alg == QA_ALG_BRUTE_FORCE) {
+        if (std::pow((double)n_max + 1.0, (double)n) >= 4.611686018427388e18) return QA_ERR_OVERFLOW;
+        if (closed && (int64_t)n * n_max < N_hat) return QA_ERR_INFEASIBLE;
+    }
+    if (P == 0) return QA_OK;
+    if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
+    if (!d_ws || ws_bytes < carve(m, P, nullptr, nullptr) || (reinterpret_cast<uintptr_t>(d_ws) & 255u))
+        return QA_ERR_INVALID_ARG;
+    QaWorkspace ws;
+    carve(m, P, d_ws, &ws);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1};
+    g_n_marks = 0;
+    timing_mark(stream);
+    QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, nullptr, d_stats, stream));
+    timing_mark(stream);
+    const double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n)
+                          : alg == QA_ALG_DEFAULT   ? std::pow(2.0, (double)n)
+                                                    : std::pow(1.0 + t, (double)n);
+    QA_CUDA(qa_launch_thermal(m->dev, n, ws, a, kT, expect, d_Nmean, d_Emin, d_stats, stream));
+    timing_mark(stream);
+    return QA_OK;
+}
+
 }  // namespace
 
 void qa_timing_mark(cudaStream_t stream) { timing_mark(stream); }
@@ -467,6 +504,21 @@ qa_status qa_ground_state_host(const qa_model *mc, const double *h_Vg, int64_t P
     if (e != cudaSuccess) return cuda_fail(e, "qa_ground_state_host");
     if (e2 != cudaSuccess) return cuda_fail(e2, "qa_ground_state_host sync");
     return QA_OK;
+}
+
+qa_status qa_thermal_open(const qa_model *m, const double *d_Vg, int64_t P, qa_algorithm alg, double t, int n_max, double kT,
+                          double *d_Nmean, double *d_Emin, qa_stats *d_stats, void *d_workspace, size_t workspace_bytes,
+                          void *cuda_stream)
+{
+    return thermal(m, d_Vg, P, 0, 0, alg, t, n_max, kT, d_Nmean, d_Emin, d_stats, d_workspace, workspace_bytes, cuda_stream);
+}
+
+qa_status qa_thermal_closed(const qa_model *m, const double *d_Vg, int64_t P, int N_hat, qa_algorithm alg, double t, int n_max,
+                            double kT, double *d_Nmean, double *d_Emin, qa_stats *d_stats, void *d_workspace,
+                            size_t workspace_bytes, void *cuda_stream)
+{
+    return thermal(m, d_Vg, P, 1, N_hat, alg, t, n_max, kT, d_Nmean, d_Emin, d_stats, d_workspace, workspace_bytes,
+                   cuda_stream);
 }
 
 qa_status qa_batch_create(const qa_model *const *models, int n_models, qa_batch **out)

@@ -203,6 +203,69 @@ def test_general_spd_matrices(api, n):
             check(api, w, algorithm="brute", n_max=3)
 
 
+# ---- thermal broadening, Eq. (10): mean occupation vs the oracle ----------------------------
+def check_thermal(api, w, kT_over_EC, **kw):
+    m = api.Model(w.C_dd, w.C_gd)
+    om = oracle.Model(w.C_dd, w.C_gd)
+    kT = kT_over_EC * om.EC
+    r = m.thermal(torch.from_numpy(w.Vg).cuda(), kT, regime=w.regime, N_hat=w.N_hat, want_stats=True, **kw)
+    torch.cuda.synchronize()
+    okw = dict(kw)
+    if okw.get("algorithm") == "brute_force":
+        okw["algorithm"] = "brute"
+    o = om.thermal(w.Vg, kT, regime=w.regime, N_hat=w.N_hat, **okw)
+    Nm, Em = r["Nmean"].cpu().numpy(), r["Emin"].cpu().numpy()
+    # tolerance: the incremental energies drift by <~ 1e-13 E_C over a walk, i.e. 1e-13 E_C / kT in a weight
+    tol = 1e-9 * max(1.0, 0.02 / kT_over_EC)
+    assert np.abs(Nm - o["Nmean"]).max() <= tol * max(1.0, np.abs(o["Nmean"]).max())
+    fin = np.isfinite(o["Emin"])
+    assert np.abs(Em[fin] - o["Emin"][fin]).max() <= 1e-9 * max(om.EC, np.abs(o["Emin"][fin]).max())
+    assert api.stats_dict(r["stats"])["n_candidates_scored"] == int(o["n_scored"].sum())
+    return Nm, o
+
+
+def test_thermal_small_configs(api):
+    w = wl.config1(60, 50)
+    Nm, o = check_thermal(api, w, 0.05, algorithm="default")
+    assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_kernel<G=1>"]
+    assert ((Nm > 0.01) & (Nm < 0.99)).any()          # transitions are actually broadened
+    check_thermal(api, w, 0.3, algorithm="brute", n_max=5)
+    w2 = wl.config2(40, 30)
+    Nm, o = check_thermal(api, w2, 0.05, algorithm="default")
+    assert np.allclose(Nm.sum(1), 5.0, atol=1e-9)     # closed array: the total charge survives the average
+    check_thermal(api, w2, 0.2, algorithm="thresholded", t=0.3)
+    check_thermal(api, w2, 0.1, algorithm="brute", n_max=5)
+    assert api.last_launch_plan()[0][1] == "qa_thermal_kernel<G=256>"
+
+
+@pytest.mark.parametrize("n,P", [(1, 300), (4, 300), (8, 257), (11, 65), (13, 9), (16, 5)])
+def test_thermal_all_sizes(api, n, P):
+    w = wl.random_open(n, n, P, seed=600 + n, lo=-0.4, hi=2.6)
+    check_thermal(api, w, 0.08, algorithm="default")
+    check_thermal(api, w, 0.5, algorithm="thresholded", t=0.4)
+    if n <= 11:
+        w.regime, w.N_hat = "closed", max(1, n)
+        check_thermal(api, w, 0.08, algorithm="default")
+
+
+def test_thermal_cold_limit_is_the_ground_state_and_errors(api):
+    w = wl.config5_array(1, 40, 40)
+    m = api.Model(w.C_dd, w.C_gd)
+    Vg = torch.from_numpy(w.Vg).cuda()
+    g = m.ground_state(Vg)
+    _, EC = m.inverse()
+    c = m.thermal(Vg, 1e-5 * EC)
+    om = oracle.Model(w.C_dd, w.C_gd)
+    o = om.ground_state(w.Vg)
+    clear = torch.from_numpy(o["E2"] - o["E"] > 1e-2 * EC).cuda()
+    assert clear.sum() > 1000
+    assert torch.allclose(c["Nmean"][clear], g["N"][clear].double(), atol=1e-9)
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(api.QaError) as e:
+            m.thermal(Vg, bad)
+        assert e.value.status == 1
+
+
 # ---- dataset batch: one launch over several models == a loop over the single-model call ------------------------------
 def test_batch_equals_loop_and_oracle(api):
     wls = [wl.config5_array(j, 40, 33) for j in range(5)]
