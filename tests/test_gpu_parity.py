@@ -227,7 +227,7 @@ def check_thermal(api, w, kT_over_EC, **kw):
 def test_thermal_small_configs(api):
     w = wl.config1(60, 50)
     Nm, o = check_thermal(api, w, 0.05, algorithm="default")
-    assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_kernel<G=1>"]
+    assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_gray_kernel<G=1>"]
     assert ((Nm > 0.01) & (Nm < 0.99)).any()          # transitions are actually broadened
     check_thermal(api, w, 0.3, algorithm="brute", n_max=5)
     w2 = wl.config2(40, 30)
