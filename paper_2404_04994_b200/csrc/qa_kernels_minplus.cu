@@ -8,12 +8,16 @@
 // h_i = [M d0]_i + 1/2 M_ii (prologue) and h'_j = h_j + sum_{jh in t} M[j][jh], the energy (C1) L607 separates as
 //     e(t,u,w) = A[u] + ( B[w] + QL[u,w] )
 //     B[w]     = offW + sum_{j in w} h'_j                 2^NW values, registers, built once per (thread, pixel)
-//     A[u]     = be + offU + sum_{j in u} h'_j            one DADD per u (prefix sums over the bits of u)
+//     A[u]     = be + offU + sum_{j in u} h'_j            (bits of u >> 2 added from the highest down, then {0, h'_NW, h'_NW+1, sum})
 //     QL[u,w]  = pair energy sum_{j<j' in (u,w)} M_jj'    pixel- and thread-independent: kernel parameter (constant bank)
-//     be       = E(base) + E_C + pairs(t) + sum_{jh in t} h_jh        offW = E_C + sum_{j<NW} |h_j|,  offU = sum_{j>=NW} |h_j|
-// so that  min_w e = A[u] + min_w (B[w] + QL[u,w]):  per candidate ONE DADD  y = B[w] + QL[u,w]  (register + constant
-// operand, static addresses because the loops are fully unrolled) and half an integer min3 on the high words.  The
-// offsets make every y and every A positive, so the high 32 bits of the fp64 pattern order like the values.
+//     be       = E(base) + QHT[t] + sum_{jh in t} h_jh    offW = E_C + sum_{j<NW} |h_j|,  offU = sum_{j>=NW} |h_j|
+// (VT[t][j] = the cross term of t with low bit j and QHT[t] = E_C + pairs(t) are model tables, qa_api.cu rebuild), so that
+// min_w e = A[u] + min_w (B[w] + QL[u,w]):  per candidate ONE DADD  y = B[w] + QL[u,w]  and half an integer min3 on the high
+// words.  The offsets make every y and every A positive, so the high 32 bits of the fp64 pattern order like the values; they
+// are thread-independent (the bounds L_t are compared across the threads of a pixel).  Table entries reach the DADD through
+// uniform registers: a real loop over chunks of 4 u (64 entries) keeps the address "uniform register + immediate"
+// (LDCU.64; measured: one indexed LDCU per ~4 cycles per scheduler), and every entry serves the PX = 2 pixels a thread
+// walks at once.  DESIGN.md section 6 lists what else was measured (register-bank conflicts of the min3, LDS vs LDCU).
 //
 //   qa_minplus_walk_kernel (pass 1; a lower bound per thread):
 //       m_u  = min_w hi32(y)                               (ALU pipe, VIMNMX3)
@@ -30,8 +34,8 @@
 //     orders of magnitude below the 1e-9 E_C near-tie rule.  The same warp then decodes N* and recomputes E(N*) from the
 //     definition (S7), so the path is three launches: prologue, walk, finish.
 //
-// FP64-pipe instructions per (thread, pixel): 2^NL (y) + 2*2^NU (A, LB) + 2^NW - 1 (B) + 2 NL (h', offsets) + NH + 1 (be)
-// = 327 per 256 candidates at NU = NW = 4, i.e. 1.28 per candidate (the filtered Gray walk it replaces: 2.06).
+// FP64-pipe instructions per (thread, pixel) at NU = NW = 4, NH = 8: 256 (y) + 20 (A) + 16 (LB) + 15 (B) + 8 (h') + 8
+// (offsets) + 11 (be, a0, lo3) = 334 per 256 candidates, i.e. 1.30 per candidate (exact-compare Gray walk: 3).
 //
 // Index convention as in qa_kernels_walk.cu: candidate index = sum_i b_i 2^(n-1-i) = (t << NL) | (u << NW) | w.
 #include "qa_internal.cuh"
