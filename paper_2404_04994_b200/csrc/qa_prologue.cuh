@@ -132,6 +132,36 @@ __device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool 
             if (closed) failed = true;
             break;
         }
+        if (!general && !closed && __popc(A) <= 2) {
+            // one or two clamped dots of an open array (nearly every QP pixel of a sweep): the 1x1 / 2x2 system in closed
+            // form, registers only -- y_A = -C_AA^-1 c_A, x_F = c_F + C_FA y_A
+            const int ia = __ffs(A) - 1;
+            const unsigned A2 = A & (A - 1);
+            const int ib = A2 ? __ffs(A2) - 1 : ia;
+            double ca = 0.0, cb = 0.0;
+#pragma unroll
+            for (int f = 0; f < N; ++f) {
+                if (f == ia) ca = c[f];
+                if (f == ib) cb = c[f];
+            }
+            double ya, yb = 0.0;
+            if (A2) {
+                const double Caa = sC[ia * N + ia], Cab = sC[ia * N + ib], Cbb = sC[ib * N + ib];
+                const double det = Caa * Cbb - Cab * Cab;
+                ya = (cb * Cab - ca * Cbb) / det;
+                yb = (ca * Cab - cb * Caa) / det;
+            } else {
+                ya = -ca / sC[ia * N + ia];
+            }
+            if (ya < -1e-9 * scale || yb < -1e-9 * scale) failed = true;  // KKT: bound multipliers must be >= 0
+#pragma unroll
+            for (int f = 0; f < N; ++f) {
+                double s = c[f] + sC[f * N + ia] * ya;
+                if (A2) s += sC[f * N + ib] * yb;
+                x[f] = ((A >> f) & 1u) ? 0.0 : s;  // clamped components are exactly 0 (R3)
+            }
+            continue;
+        }
         qa_qp_eqp<N>(sC, c, closed, Nhat, A, x, r);
         if (!general)
             for (int i = 0; i < N; ++i)
