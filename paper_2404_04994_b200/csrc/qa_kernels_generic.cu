@@ -103,6 +103,8 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
     __shared__ uint64_t sI[ENUM_THREADS / 32];
     for (int e = threadIdx.x; e < N * N; e += ENUM_THREADS) sM[e] = mdl->M[(e / N) * QA_MAXN + (e % N)];
     __syncthreads();
+    qa_pdl_launch_dependents();
+    qa_pdl_wait();  // M is model data; everything below was written by the prologue kernel
 
     const int64_t P = ws.P;
     const int64_t p = (blockIdx.x * (int64_t)ENUM_THREADS + threadIdx.x) / G;
@@ -216,6 +218,7 @@ __global__ void __launch_bounds__(FIN_THREADS) qa_finalize_kernel(const QaDevMod
                                                                   double *__restrict__ outVs)
 {
     const int64_t p = blockIdx.x * (int64_t)FIN_THREADS + threadIdx.x;
+    qa_pdl_wait();  // ws.best comes from the candidate kernel launched just before
     if (p >= ws.P) return;
     qa_finalize_pixel(mdl, Vg, ws, p, ws.best[p], outN, outE, outVs);
 }
@@ -256,19 +259,21 @@ template <int N>
 cudaError_t launch_enumerate_n(const QaDevModel *d_model, QaWorkspace ws, QaCallArgs args, double expect_cand,
                                qa_stats *d_stats, cudaStream_t stream)
 {
+    cudaError_t err;
     if (expect_cand <= 64.0) {
         const unsigned blocks = (unsigned)((ws.P + ENUM_THREADS - 1) / ENUM_THREADS);
-        qa_enumerate_kernel<N, 1><<<blocks, ENUM_THREADS, 0, stream>>>(d_model, ws, args, d_stats);
+        err = qa_launch_pdl(qa_enumerate_kernel<N, 1>, dim3(blocks), dim3(ENUM_THREADS), stream, d_model, ws, args, d_stats);
         qa_plan_add("qa_enumerate_kernel<G=1>");
     } else if (expect_cand <= 4096.0) {
         const unsigned blocks = (unsigned)((ws.P * 32 + ENUM_THREADS - 1) / ENUM_THREADS);
-        qa_enumerate_kernel<N, 32><<<blocks, ENUM_THREADS, 0, stream>>>(d_model, ws, args, d_stats);
+        err = qa_launch_pdl(qa_enumerate_kernel<N, 32>, dim3(blocks), dim3(ENUM_THREADS), stream, d_model, ws, args, d_stats);
         qa_plan_add("qa_enumerate_kernel<G=32>");
     } else {
-        qa_enumerate_kernel<N, ENUM_THREADS><<<(unsigned)ws.P, ENUM_THREADS, 0, stream>>>(d_model, ws, args, d_stats);
+        err = qa_launch_pdl(qa_enumerate_kernel<N, ENUM_THREADS>, dim3((unsigned)ws.P), dim3(ENUM_THREADS), stream, d_model, ws,
+                            args, d_stats);
         qa_plan_add("qa_enumerate_kernel<G=256>");
     }
-    return cudaGetLastError();
+    return err;
 }
 
 }  // namespace
@@ -318,8 +323,7 @@ cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, Qa
     (void)d_stats;
     qa_plan_add("qa_finalize_kernel");
     const unsigned blocks = (unsigned)((ws.P + FIN_THREADS - 1) / FIN_THREADS);
-    qa_finalize_kernel<<<blocks, FIN_THREADS, 0, stream>>>(d_model, d_Vg, ws, d_N, d_E, d_Vsensor);
-    return cudaGetLastError();
+    return qa_launch_pdl(qa_finalize_kernel, dim3(blocks), dim3(FIN_THREADS), stream, d_model, d_Vg, ws, d_N, d_E, d_Vsensor);
 }
 
 cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int iters, cudaStream_t stream)

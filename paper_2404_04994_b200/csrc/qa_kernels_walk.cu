@@ -65,6 +65,8 @@ __global__ void __launch_bounds__(WALK_THREADS) qa_walk_kernel(const QaDevModel 
         for (int jh2 = jh + 1; jh2 < NH; ++jh2)
             if (((t >> jh) & 1u) && ((t >> jh2) & 1u)) QH += mdl->M[(N - 1 - NL - jh) * QA_MAXN + (N - 1 - NL - jh2)];
 
+    qa_pdl_launch_dependents();
+    qa_pdl_wait();  // the constants above are model data; h comes from the prologue kernel
     const int64_t groups = (P + PPC - 1) / PPC;
     int buf = 0;
     for (int64_t grp = blockIdx.x; grp < groups; grp += gridDim.x, buf ^= 1) {
@@ -147,8 +149,7 @@ cudaError_t launch_walk(const QaDevModel *d_model, const QaWalkTable &tab, QaWor
     if (per_sm < 1) per_sm = 1;
     int64_t grid = (int64_t)sm_count * per_sm;
     if (grid > groups) grid = groups;
-    qa_walk_kernel<NL, NH><<<(unsigned)grid, WALK_THREADS, 0, stream>>>(d_model, tab, ws);
-    return cudaGetLastError();
+    return qa_launch_pdl(qa_walk_kernel<NL, NH>, dim3((unsigned)grid), dim3(WALK_THREADS), stream, d_model, tab, ws);
 }
 
 }  // namespace
