@@ -390,6 +390,24 @@ def test_full_size_config4_sampled(api):
     assert (np.where(dn_ok, -grad + half, 1.0) >= -1e-9).all()
 
 
+def test_full_size_config5_batch_call_sampled(api):
+    """The launch configuration bench.py --workload config5 times (qa_ground_state_batch over full 128x128 members),
+    on 16 members: sampled pixels of every member against the oracle, all three algorithms."""
+    B = 16
+    wls = [wl.config5_array(j) for j in range(B)]
+    batch = api.Batch([api.Model(w.C_dd, w.C_gd) for w in wls])
+    Vg = torch.from_numpy(np.stack([w.Vg for w in wls])).cuda()
+    rng = np.random.default_rng(3)
+    for kw in (dict(algorithm="default"), dict(algorithm="thresholded", t=0.2), dict(algorithm="thresholded", t=0.5)):
+        r = batch.ground_state(Vg, **kw)
+        N, E = r["N"].cpu().numpy(), r["E"].cpu().numpy()
+        assert (N >= 0).all()
+        for j, w in enumerate(wls):
+            sel = np.sort(rng.choice(w.P, size=250, replace=False))
+            om = oracle.Model(w.C_dd, w.C_gd)
+            compare(N[j][sel], E[j][sel], om.ground_state(w.Vg[sel], **kw), om.EC)
+
+
 def test_full_size_config5_batch_member_sampled(api):
     w = wl.config5_array(3)
     m = api.Model(w.C_dd, w.C_gd)
