@@ -184,8 +184,9 @@ QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernel
 
 /* Kernel selection (process-wide; cross-check aid, the results are identical): 0 = the three-kernel path for every n_dot
  * (prologue, exact-compare Gray walk or enumeration, finalize), 1 (default) = the min-plus walk with its finish kernel for
- * the open default search of n_dot >= 13 and the one-kernel path for n_dot <= 8.  Returns
- * QA_ERR_INVALID_ARG for any other value. */
+ * the open default search of n_dot >= 13 and the one-kernel path for n_dot <= 8, 2 = as 1, but the
+ * open default search of n_dot >= 13 skips the high patterns a rigorous lower bound excludes (same arg min; fewer
+ * candidates are scored explicitly).  Returns QA_ERR_INVALID_ARG for any other value. */
 QA_API qa_status qa_set_walk_variant(int variant);
 
 /* Names of the kernels the last ground-state call on this host thread enqueued (comma separated; static storage). */

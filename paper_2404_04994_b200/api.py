@@ -340,7 +340,8 @@ def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch
 
 
 def set_walk_variant(variant: int) -> None:
-    """qa_set_walk_variant: 0 = exact-compare Gray walk, 1 = min-plus walk (default) for n_dot >= 13 (cross-check aid)."""
+    """qa_set_walk_variant: 0 = three-kernel path everywhere, 1 = default (min-plus walk for n_dot >= 13, one-kernel path
+    for n_dot <= 8), 2 = as 1 with exact pruning of the high patterns in the min-plus walk."""
     _check(lib().qa_set_walk_variant(int(variant)), "qa_set_walk_variant")
 
 

@@ -160,6 +160,7 @@ qa_status rebuild(qa_model *m)
                 for (int jh = 0; jh < NH; ++jh)
                     if ((t >> jh) & 1) s += Msub[(n - 1 - j) * n + (n - 1 - NL - jh)];
                 h.VT[t * NL + j] = s;
+                h.VTt[j * (1 << QA_WALK_NL) + t] = s;
             }
             double q = h.EC;
             for (int jh = 0; jh < NH; ++jh)
@@ -182,7 +183,7 @@ int walk_variant()
     if (g_walk_variant < 0) {
         const char *e = std::getenv("QA_WALK_VARIANT");
         g_walk_variant = e ? std::atoi(e) : 1;
-        if (g_walk_variant < 0 || g_walk_variant > 1) g_walk_variant = 1;
+        if (g_walk_variant < 0 || g_walk_variant > 2) g_walk_variant = 1;
     }
     return g_walk_variant;
 }
@@ -207,6 +208,7 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
     uint64_t *be = static_cast<uint64_t *>(take(Pz * 8));
     double *e0 = static_cast<double *>(take(Pz * 8));
     uint2 *rec = static_cast<uint2 *>(take(n >= 13 ? Pz * 8 * ((size_t)1 << (n - 13)) : 0));
+    unsigned long long *counter = static_cast<unsigned long long *>(take(256));
     if (ws) {
         ws->h = h;
         ws->nc = nc;
@@ -216,6 +218,7 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
         ws->best = be;
         ws->e0 = e0;
         ws->rec = rec;
+        ws->counter = counter;
         ws->P = P;
     }
     return off;
@@ -260,7 +263,8 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd
     if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && walk_variant() != 0 && m->is_z) {
         const bool fuse = m->ns == 0;  // S7 runs inside the finish kernel: no finalize launch
-        QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count, stream));
+        QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count,
+                                       walk_variant() == 2, stream));
         timing_mark(stream);
         if (fuse) return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && !closed) {
@@ -640,7 +644,7 @@ qa_status qa_set_kernel_timing(int enable)
 
 qa_status qa_set_walk_variant(int variant)
 {
-    if (variant < 0 || variant > 1) return QA_ERR_INVALID_ARG;
+    if (variant < 0 || variant > 2) return QA_ERR_INVALID_ARG;
     g_walk_variant = variant;
     return QA_OK;
 }

@@ -39,6 +39,7 @@ struct QaDevModel {
     //   QHT[t]   = E_C + sum_{jh<jh' in t} M[n-1-NL-jh][n-1-NL-jh']                       pair energy of t, plus E_C
     double VT[(1 << QA_WALK_NL) * QA_WALK_NL];
     double QHT[1 << QA_WALK_NL];
+    double VTt[QA_WALK_NL * (1 << QA_WALK_NL)];  // VT transposed, [j][t]: coalesced when the lanes hold consecutive t
 };
 
 // Per-call scratch, structure-of-arrays over pixels ([i][P] so that thread-per-pixel accesses coalesce).
@@ -50,6 +51,7 @@ struct QaWorkspace {
     uint64_t *total;  // [P]     product of cnt = size of the enumerated set
     uint64_t *best;   // [P]     mixed-radix index (dot 0 most significant) of the argmin, ~0 if the set is empty
     double *e0;       // [P]     E(base) = 1/2 (base - N_c)^T M (base - N_c) >= 0, the energy of the base point
+    unsigned long long *counter;  // work counter of the pruned min-plus walk (zeroed by the prologue kernel)
     uint2 *rec;       // [P][2^(n-13)]  min-plus walk: per warp of the pixel (min of L over its lanes, ballot of lanes near it)
     int64_t P;
 };
@@ -82,7 +84,7 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
 cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, qa_stats *d_stats,
                            int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
-                                   double *d_E, int sm_count, cudaStream_t stream);
+                                   double *d_E, int sm_count, int pruned, cudaStream_t stream);
 cudaError_t qa_launch_fused_small(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
                                   QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats,
                                   cudaStream_t stream);

@@ -33,6 +33,7 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
     const double oneC1 = mdl->oneC1;
     __syncthreads();
     qa_pdl_launch_dependents();  // the candidate kernel may become resident and load its constants meanwhile
+    if (blockIdx.x == 0 && threadIdx.x == 0) *ws.counter = 0ull;  // work counter of the pruned min-plus walk
 
     const int64_t P = ws.P;
     const int64_t p = blockIdx.x * (int64_t)PRO_THREADS + threadIdx.x;

@@ -271,6 +271,181 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
+// pass 1 with exact pruning (opt-in: qa_set_walk_variant(2)).  One WARP owns a pair of pixels.
+//   bound:   every high pattern t gets LB_t = be_t + sum_{j low} min(0, h'_j) <= every e(t, ., .) (the pair energies are
+//            >= 0 because M >= 0 for a Maxwell c_dd), and UB = min_t (LB_t + QL[b_t]), b_t = {j : h'_j < 0}: the energy of a
+//            real candidate.  A pattern with LB_t > UB cannot hold the argmin (nor a tie of it).
+//   compact: the surviving patterns of the pixel (7 % of the 256 on config 4) are listed in shared memory;
+//   walk:    32 of them at a time, one per lane, through the same chunk loop as qa_minplus_walk_kernel (the pair table
+//            is lane-independent; VT[t], QHT[t] are gathered per lane);
+//   record:  the per-pattern bounds L_t are turned into the same per-32-patterns records (minimum, ballot) the full
+//            walk writes, so qa_minplus_finish_kernel runs unchanged.
+// Same argmin as the full enumeration; the candidates of the pruned patterns are covered by the bound, not scored.
+template <int NH, int NU, int NW, int MINB>
+__global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_pruned_kernel(const QaDevModel *__restrict__ mdl,
+                                                                             const __grid_constant__ MpTable<NU + NW> tab,
+                                                                             QaWorkspace ws)
+{
+    constexpr int PX = 2;
+    constexpr int NL = NU + NW;
+    constexpr int N = NL + NH;
+    constexpr int TP = 1 << NH;          // high patterns per pixel
+    constexpr int KP = TP / 32;          // patterns per lane in the bound phase = records per pixel
+    constexpr int NCH = 1 << (NU - 2);
+    constexpr int WARPS = MP_THREADS / 32;
+    static_assert(NH >= 5 && NH <= 8 && NW >= 2 && NU >= 2, "whole groups of 32 patterns");
+    __shared__ unsigned sL[WARPS][PX][TP];        // L_t of every pattern (0xffffffff: pruned)
+    __shared__ unsigned char sList[WARPS][PX][TP];  // surviving patterns
+
+    const unsigned lane = threadIdx.x & 31u;
+    const int wid = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);  // warp-uniform, and ptxas can see it
+    const int64_t P = ws.P;
+    const double EC = mdl->EC;
+    const int64_t groups = (P + PX - 1) / PX;
+    const int64_t nwarps = (int64_t)gridDim.x * WARPS;
+    qa_pdl_launch_dependents();
+    qa_pdl_wait();
+
+    // pixel pairs are handed out through a counter (zeroed by the prologue kernel): the survivors per pixel vary
+    (void)nwarps;
+    for (;;) {
+        long long take = 0;
+        if (lane == 0) take = (long long)atomicAdd(reinterpret_cast<unsigned long long *>(ws.counter), 1ull);
+        const int64_t grp = __shfl_sync(0xffffffffu, take, 0);
+        if (grp >= groups) break;
+        double myv[PX];
+        int S[PX];
+#pragma unroll
+        for (int px = 0; px < PX; ++px) {
+            int64_t p = grp * PX + px;
+            if (p >= P) p = P - 1;
+            myv[px] = 0.0;
+            if (lane <= N) myv[px] = lane < N ? __ldg(ws.h + (int64_t)lane * P + p) : __ldg(ws.e0 + p);
+            // ---- bound phase: lane handles the patterns t = 32 k + lane
+            double hl[NL], hh[NH];
+#pragma unroll
+            for (int j = 0; j < NL; ++j) hl[j] = mp_shfl(myv[px], N - 1 - j);
+#pragma unroll
+            for (int jh = 0; jh < NH; ++jh) hh[jh] = mp_shfl(myv[px], N - 1 - NL - jh);
+            const double e0 = mp_shfl(myv[px], N);
+            double LBk[KP], ub = INFINITY;
+#pragma unroll
+            for (int k = 0; k < KP; ++k) {
+                const unsigned t = (unsigned)k * 32u + lane;
+                double lb = e0 + mdl->QHT[t];
+#pragma unroll
+                for (int jh = 0; jh < NH; ++jh)
+                    if ((t >> jh) & 1u) lb += hh[jh];
+                unsigned bl = 0;
+#pragma unroll
+                for (int j = 0; j < NL; ++j) {
+                    const double hpj = hl[j] + mdl->VTt[j * (1 << QA_WALK_NL) + t];
+                    if (hpj < 0.0) {
+                        lb += hpj;
+                        bl |= 1u << j;
+                    }
+                }
+                LBk[k] = lb;
+                ub = fmin(ub, lb + mdl->QL[bl]);
+                sL[wid][px][t] = 0xffffffffu;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) ub = fmin(ub, mp_shfl(ub, (int)(lane ^ o)));
+            ub += 1e-9 * EC;  // rounding of the bounds is ~1e-15 relative; the margin keeps every tie of the minimum
+            // ---- compaction
+            int cnt = 0;
+#pragma unroll
+            for (int k = 0; k < KP; ++k) {
+                const bool keep = LBk[k] <= ub;
+                const unsigned bal = __ballot_sync(0xffffffffu, keep);
+                if (keep) sList[wid][px][cnt + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)(k * 32 + lane);
+                cnt += __popc(bal);
+            }
+            S[px] = cnt;  // >= 1: the pattern attaining ub is kept
+        }
+        __syncwarp();
+        // ---- walk the survivors, 32 at a time
+        const int rounds = __shfl_sync(0xffffffffu, (max(S[0], S[1]) + 31) >> 5, 0);
+#pragma unroll 1
+        for (int rd = 0; rd < rounds; ++rd) {
+            double B[PX][1 << NW], hu[PX][NU], a0[PX], lo3[PX];
+            unsigned tt[PX];
+            bool valid[PX];
+#pragma unroll
+            for (int px = 0; px < PX; ++px) {
+                const int idx = rd * 32 + (int)lane;
+                valid[px] = idx < S[px];
+                const unsigned t = sList[wid][px][valid[px] ? idx : 0];
+                tt[px] = t;
+                double hw[NW], offw = EC, offu = 0.0;
+#pragma unroll
+                for (int j = 0; j < NL; ++j) {
+                    const double hj = mp_shfl(myv[px], N - 1 - j);
+                    const double hpj = hj + mdl->VT[t * NL + j];
+                    if (j < NW) {
+                        hw[j] = hpj;
+                        offw += fabs(hj);
+                    } else {
+                        hu[px][j - NW] = hpj;
+                        offu += fabs(hj);
+                    }
+                }
+                double be = mp_shfl(myv[px], N) + mdl->QHT[t];
+#pragma unroll
+                for (int jh = 0; jh < NH; ++jh) {
+                    const double hv = mp_shfl(myv[px], N - 1 - NL - jh);
+                    if ((t >> jh) & 1u) be += hv;
+                }
+                a0[px] = be + offu;
+                lo3[px] = hu[px][1] + hu[px][0];
+                B[px][0] = offw;
+#pragma unroll
+                for (int w = 1; w < (1 << NW); ++w) B[px][w] = B[px][w & (w - 1)] + hw[mp_ctz(w)];
+            }
+            unsigned L[PX];
+#pragma unroll
+            for (int px = 0; px < PX; ++px) L[px] = 0xffffffffu;
+            int iv;
+            asm volatile("mov.u32 %0, 0;" : "=r"(iv));
+#pragma unroll 1
+            for (int i = 0; i < NCH; ++i, ++iv) {
+                const double2 *q = reinterpret_cast<const double2 *>(tab.q) + (i << (NW + 1));
+                double a[4][PX];
+#pragma unroll
+                for (int px = 0; px < PX; ++px) {
+                    double ah = a0[px];
+#pragma unroll
+                    for (int j = NU - 1; j >= 2; --j)
+                        if ((iv >> (j - 2)) & 1) ah += hu[px][j];
+                    a[0][px] = ah;
+                    a[1][px] = ah + hu[px][0];
+                    a[2][px] = ah + hu[px][1];
+                    a[3][px] = ah + lo3[px];
+                }
+                mp_chunk<NW, PX>(q, B, a, L);
+            }
+#pragma unroll
+            for (int px = 0; px < PX; ++px)
+                if (valid[px]) sL[wid][px][tt[px]] = L[px];
+        }
+        __syncwarp();
+        // ---- records in the format of the full walk: one per 32 consecutive patterns
+#pragma unroll
+        for (int px = 0; px < PX; ++px) {
+            const int64_t p = grp * PX + px;
+#pragma unroll
+            for (int qd = 0; qd < KP; ++qd) {
+                const unsigned v = sL[wid][px][qd * 32 + (int)lane];
+                const unsigned wmin = __reduce_min_sync(0xffffffffu, v);
+                const unsigned ball = __ballot_sync(0xffffffffu, v != 0xffffffffu && v - wmin <= 2u);
+                if (lane == 0 && p < P) ws.rec[p * KP + qd] = make_uint2(wmin, ball);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
 // pass 2 + S7: one warp per pixel.  The code runs once per warp (10^4 warps at config 4), so what it pays for is the
 // instruction count and the MIO queue (shuffles, loads), not arithmetic: every lane loads the pixel's inputs itself
 // (warp-uniform addresses, one L1 request each) instead of trading them by shuffle, the survivor's constants come from
@@ -447,10 +622,42 @@ cudaError_t launch_mp(const QaDevModel *d_model, const double *QLhost, QaWorkspa
 
 }  // namespace
 
+template <int NH>
+cudaError_t launch_mp_pruned(const QaDevModel *d_model, const double *QLhost, QaWorkspace ws, int32_t *d_N, double *d_E,
+                             int sm_count, cudaStream_t stream)
+{
+    MpTable<8> local;
+    for (int b = 0; b < 256; ++b) local.q[b] = QLhost[b];
+    int per_sm = 0;
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_pruned_kernel<NH, 4, 4, 2>, MP_THREADS, 0);
+    if (err != cudaSuccess) return err;
+    if (per_sm < 1) per_sm = 1;
+    int64_t grid = (int64_t)sm_count * per_sm;
+    const int64_t need = ((ws.P + 1) / 2 + MP_THREADS / 32 - 1) / (MP_THREADS / 32);
+    if (grid > need) grid = need;
+    err = qa_launch_pdl(qa_minplus_pruned_kernel<NH, 4, 4, 2>, dim3((unsigned)grid), dim3(MP_THREADS), stream, d_model, local, ws);
+    if (err != cudaSuccess) return err;
+    qa_plan_add("qa_minplus_finish_kernel");
+    qa_timing_mark(stream);
+    const int64_t fblocks = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
+    return qa_launch_pdl(qa_minplus_finish_kernel<NH, 4, 4>, dim3((unsigned)fblocks), dim3(MF_THREADS), stream, d_model, ws, d_N,
+                         d_E);
+}
+
 // d_N == nullptr: the finish kernel only stores the winning index (ws.best) and the caller runs qa_finalize_kernel.
 cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
-                                   double *d_E, int sm_count, cudaStream_t stream)
+                                   double *d_E, int sm_count, int pruned, cudaStream_t stream)
 {
+    if (pruned) {
+        qa_plan_add("qa_minplus_pruned_kernel");
+        switch (n) {
+            case 13: return launch_mp_pruned<5>(d_model, QLhost, ws, d_N, d_E, sm_count, stream);
+            case 14: return launch_mp_pruned<6>(d_model, QLhost, ws, d_N, d_E, sm_count, stream);
+            case 15: return launch_mp_pruned<7>(d_model, QLhost, ws, d_N, d_E, sm_count, stream);
+            case 16: return launch_mp_pruned<8>(d_model, QLhost, ws, d_N, d_E, sm_count, stream);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     qa_plan_add("qa_minplus_walk_kernel");
 #define MP_CALL(NH) launch_mp<NH, 4, 4, 2, 2>(d_model, QLhost, ws, d_N, d_E, sm_count, stream)
     switch (n) {

@@ -103,18 +103,20 @@ def test_config4_open_grid16_default(api, W, H):
 
 @pytest.mark.parametrize("n,P", [(13, 45), (14, 46), (15, 33), (16, 45), (16, 1)])
 def test_walk_variants_agree(api, n, P):
-    """The exact-compare Gray walk (variant 0) and the min-plus walk + finish kernel (variant 1, the default for
-    n >= 13) give the same charge map and the same energies up to the summation order of E(N*); each is also checked
-    against the oracle.  P odd / P = 1: the ragged last pixel pair of the min-plus walk."""
+    """The exact-compare Gray walk (variant 0), the min-plus walk + finish kernel (variant 1, the default for n >= 13)
+    and the min-plus walk with exact pruning of the high patterns (variant 2) give the same charge map and the same
+    energies up to the summation order of E(N*); each is also checked against the oracle.  P odd / P = 1: the ragged
+    last pixel pair of the min-plus walks."""
     w = wl.random_open(n, n, P, seed=200 + n)
     ref = None
+    plans = {0: ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"],
+             1: ["qa_prologue_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"],
+             2: ["qa_prologue_kernel", "qa_minplus_pruned_kernel", "qa_minplus_finish_kernel"]}
     try:
-        for variant in (0, 1):
+        for variant in (0, 1, 2):
             api.set_walk_variant(variant)
             rep, g, o = check(api, w, algorithm="default")
-            names = g["plan"][0]
-            assert names == (["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"] if variant == 0 else
-                             ["qa_prologue_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"])
+            assert g["plan"][0] == plans[variant]
             if ref is None:
                 ref = g
             else:
@@ -131,7 +133,7 @@ def test_minplus_walk_extreme_inputs(api):
     Vg = np.concatenate([w.Vg, -50.0 * np.abs(rng.standard_normal((7, 16))), w.Vg[:9] * 40.0, np.zeros((3, 16))])
     w.Vg, w.W, w.H = np.ascontiguousarray(Vg), Vg.shape[0], 1
     try:
-        for variant in (0, 1):
+        for variant in (0, 1, 2):
             api.set_walk_variant(variant)
             check(api, w, algorithm="default")
     finally:
@@ -365,10 +367,16 @@ def test_deterministic_across_runs_and_streams(api):
 
 
 # ---- full BASELINE.json sizes in bench.py's launch configuration: sampled outputs + properties ---------------------
-def test_full_size_config4_sampled(api):
+@pytest.mark.parametrize("variant", [1, 2])
+def test_full_size_config4_sampled(api, variant):
     w = wl.config4(100, 100)
     m = api.Model(w.C_dd, w.C_gd)
-    r = m.ground_state(torch.from_numpy(w.Vg).cuda(), want_xcont=True)
+    api.set_walk_variant(variant)
+    try:
+        r = m.ground_state(torch.from_numpy(w.Vg).cuda(), want_xcont=True)
+        torch.cuda.synchronize()
+    finally:
+        api.set_walk_variant(1)
     N, E, x = r["N"].cpu().numpy(), r["E"].cpu().numpy(), r["xcont"].cpu().numpy()
     assert (N >= 0).all() and (N - np.floor(x) >= 0).all() and (N - np.floor(x) <= 1).all()
     rng = np.random.default_rng(0)
