@@ -303,6 +303,13 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_pruned_kernel(con
     const double EC = mdl->EC;
     const int64_t groups = (P + PX - 1) / PX;
     const int64_t nwarps = (int64_t)gridDim.x * WARPS;
+    // cross terms of the pattern t = 32 k + lane with low bit j: VT[t][j] = VT[lane][j] + VT[32 k][j]
+    __shared__ double sVTk[KP][NL];
+    for (int e = threadIdx.x; e < KP * NL; e += MP_THREADS) sVTk[e / NL][e % NL] = mdl->VT[((e / NL) << 5) * NL + (e % NL)];
+    double vl[NL];
+#pragma unroll
+    for (int j = 0; j < NL; ++j) vl[j] = mdl->VT[lane * NL + j];
+    __syncthreads();
     qa_pdl_launch_dependents();
     qa_pdl_wait();
 
@@ -321,25 +328,34 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_pruned_kernel(con
             if (p >= P) p = P - 1;
             myv[px] = 0.0;
             if (lane <= N) myv[px] = lane < N ? __ldg(ws.h + (int64_t)lane * P + p) : __ldg(ws.e0 + p);
-            // ---- bound phase: lane handles the patterns t = 32 k + lane
-            double hl[NL], hh[NH];
+            // ---- bound phase: lane handles the patterns t = 32 k + lane.  Both the cross terms and the high-bit sums split
+            // into a lane part (bits 0..4 of t; vl, per kernel / hlane, per pixel) and a k part (bits 5.., uniform: sVTk, hk)
+            double hb[NL];
 #pragma unroll
-            for (int j = 0; j < NL; ++j) hl[j] = mp_shfl(myv[px], N - 1 - j);
+            for (int j = 0; j < NL; ++j) hb[j] = mp_shfl(myv[px], N - 1 - j) + vl[j];
+            double hk[KP], blane = mp_shfl(myv[px], N);
 #pragma unroll
-            for (int jh = 0; jh < NH; ++jh) hh[jh] = mp_shfl(myv[px], N - 1 - NL - jh);
-            const double e0 = mp_shfl(myv[px], N);
+            for (int k = 0; k < KP; ++k) hk[k] = 0.0;
+#pragma unroll
+            for (int jh = 0; jh < NH; ++jh) {
+                const double hv = mp_shfl(myv[px], N - 1 - NL - jh);
+                if (jh < 5) {
+                    if ((lane >> jh) & 1u) blane += hv;
+                } else {
+#pragma unroll
+                    for (int k = 0; k < KP; ++k)
+                        if ((k >> (jh - 5)) & 1) hk[k] += hv;
+                }
+            }
             double LBk[KP], ub = INFINITY;
 #pragma unroll
             for (int k = 0; k < KP; ++k) {
                 const unsigned t = (unsigned)k * 32u + lane;
-                double lb = e0 + mdl->QHT[t];
-#pragma unroll
-                for (int jh = 0; jh < NH; ++jh)
-                    if ((t >> jh) & 1u) lb += hh[jh];
+                double lb = (blane + hk[k]) + mdl->QHT[t];
                 unsigned bl = 0;
 #pragma unroll
                 for (int j = 0; j < NL; ++j) {
-                    const double hpj = hl[j] + mdl->VTt[j * (1 << QA_WALK_NL) + t];
+                    const double hpj = hb[j] + sVTk[k][j];
                     if (hpj < 0.0) {
                         lb += hpj;
                         bl |= 1u << j;
