@@ -64,7 +64,9 @@ typedef struct {
     int64_t n_qp_pixels;             /* pixels whose analytic minimum had a negative component (L82-L84, L106)         */
     int64_t n_qp_rounds;             /* total active-set rounds over those pixels                                      */
     int64_t n_candidates_enumerated; /* sum over pixels of the size of the enumerated set                              */
-    int64_t n_candidates_scored;     /* ... of those whose energy entered the argmin (closed: sum N = N_hat)           */
+    int64_t n_candidates_scored;     /* ... of those whose energy entered the argmin (closed: sum N = N_hat); with the
+                                        pruned walk (qa_set_walk_variant(2)) it still counts the whole set: the pruned
+                                        candidates are covered by a bound                                              */
     int64_t n_threshold_doublings;   /* closed + thresholded: times t was doubled (L141, reading R5)                   */
     int64_t n_widened_pixels;        /* closed: floor/ceil set empty even at t = 1, set widened (reading R5)           */
     int64_t n_qp_failed;             /* pixels whose QP did not reach a KKT point (must be 0)                          */
