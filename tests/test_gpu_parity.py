@@ -126,6 +126,34 @@ def test_walk_variants_agree(api, n, P):
         api.set_walk_variant(1)
 
 
+@pytest.mark.parametrize("n", [13, 16])
+def test_minplus_walks_against_exact_walk_many_models(api, n):
+    """Many seeded models and pixels, GPU against GPU: the min-plus walks (lower-bound filter, and with pruning) must
+    return the charge state of the exact-compare walk; a differing pixel is accepted only as a near tie (energies equal
+    to 1e-9 E_C), and there must be next to none."""
+    bad = 0
+    for seed in range(10):
+        w = wl.random_open(n, n, 301, seed=900 + 17 * seed + n, lo=-0.7, hi=3.4)
+        m = api.Model(w.C_dd, w.C_gd)
+        _, EC = m.inverse()
+        Vg = torch.from_numpy(w.Vg).cuda()
+        outs = {}
+        try:
+            for variant in (0, 1, 2):
+                api.set_walk_variant(variant)
+                r = m.ground_state(Vg)
+                torch.cuda.synchronize()
+                outs[variant] = (r["N"].cpu().numpy(), r["E"].cpu().numpy())
+        finally:
+            api.set_walk_variant(1)
+        for variant in (1, 2):
+            diff = (outs[variant][0] != outs[0][0]).any(1)
+            assert np.abs(outs[variant][1] - outs[0][1])[diff].max(initial=0.0) <= 1e-9 * EC
+            assert np.allclose(outs[variant][1], outs[0][1], rtol=1e-12, atol=1e-12 * EC)
+            bad += int(diff.sum())
+    assert bad <= 2
+
+
 def test_minplus_walk_extreme_inputs(api):
     """Pixels far outside the operating range: every dot clamped (N_c << 0, huge positive h) and large occupations."""
     w = wl.config4(6, 5)
