@@ -95,7 +95,9 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
 //     E(d + delta e_i) = E(d) + delta grad_i + 1/2 delta^2 M_ii,   grad += delta M[:, i]
 // Closed arrays score only candidates with sum N = N_hat (L127, L159).  Ties: strict '<' inside a chunk keeps the
 // lexicographically first, and the cross-thread reduction is lexicographic on (E, index) (R6, on the GPU's own energies).
-template <int N, int G>
+// DEP (closed arrays): the last dot is not enumerated but set to N_hat minus the charge of the others, so only
+// prod_{i<N-1} cnt_i states are visited (brute force on config 2: 1296 instead of 7776); same states scored, same order.
+template <int N, int G, bool DEP = false>
 __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevModel *__restrict__ mdl, QaWorkspace ws,
                                                                     QaCallArgs args, qa_stats *stats)
 {
@@ -121,7 +123,8 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
         base[i] = ws.base[i * P + pp];
         cnt[i] = ws.cnt[i * P + pp];
     }
-    const uint64_t T = ws.total[pp];
+    constexpr int NE = DEP ? N - 1 : N;  // enumerated dots
+    const uint64_t T = DEP ? ws.total[pp] / (uint64_t)cnt[N - 1] : ws.total[pp];
     const uint64_t q = T / G, rem = T % G;
     const uint64_t start = r * q + (r < rem ? r : rem);
     const uint64_t len = live ? q + (r < rem ? 1 : 0) : 0;
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
     {
         uint64_t idx = start;
 #pragma unroll
-        for (int i = N - 1; i >= 0; --i) {
+        for (int i = NE - 1; i >= 0; --i) {
             const uint64_t c = (uint64_t)cnt[i];
             dg[i] = (int32_t)(idx % c);
             idx /= c;
@@ -137,10 +140,15 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
     }
     int64_t sumN = 0;
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
-        d[i] = (double)(base[i] + dg[i]) - ws.nc[i * P + pp];
-        sumN += base[i] + dg[i];
+    for (int i = 0; i < NE; ++i) sumN += base[i] + dg[i];
+    int64_t last = 0;  // DEP: the value the last dot must take (may lie outside its range: then the state is not scored)
+    if (DEP) {
+        last = (int64_t)args.N_hat - sumN;
+        dg[N - 1] = (int32_t)(last - base[N - 1]);
+        sumN = args.N_hat;
     }
+#pragma unroll
+    for (int i = 0; i < N; ++i) d[i] = (double)(base[i] + dg[i]) - ws.nc[i * P + pp];
     double E = 0.0;
 #pragma unroll
     for (int i = 0; i < N; ++i) {
@@ -156,17 +164,18 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
     uint64_t bidx = ~0ull;
     int64_t scored = 0;
     for (uint64_t it = 0; it < len; ++it) {
-        if (!closed || sumN == args.N_hat) {
+        if (DEP ? (dg[N - 1] >= 0 && dg[N - 1] < cnt[N - 1]) : (!closed || sumN == args.N_hat)) {
             ++scored;
             if (E < best) {
                 best = E;
-                bidx = start + it;
+                bidx = DEP ? (start + it) * (uint64_t)cnt[N - 1] + (uint64_t)dg[N - 1] : start + it;
             }
         }
         if (it + 1 == len) break;
-        bool carry = true;  // odometer step, least significant digit = dot N-1
+        bool carry = true;  // odometer step, least significant digit = dot NE-1
+        int dsum = 0;
 #pragma unroll
-        for (int i = N - 1; i >= 0; --i) {
+        for (int i = NE - 1; i >= 0; --i) {
             if (carry) {
                 int delta;
                 if (dg[i] == cnt[i] - 1) {
@@ -183,8 +192,17 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
 #pragma unroll
                     for (int j = 0; j < N; ++j) grad[j] = fma(dl, sM[j * N + i], grad[j]);
                     sumN += delta;
+                    dsum += delta;
                 }
             }
+        }
+        if (DEP && dsum != 0) {  // the last dot takes up the difference
+            const double dl = (double)(-dsum);
+            E += dl * (grad[N - 1] + 0.5 * dl * sM[(N - 1) * N + (N - 1)]);
+#pragma unroll
+            for (int j = 0; j < N; ++j) grad[j] = fma(dl, sM[j * N + (N - 1)], grad[j]);
+            dg[N - 1] -= dsum;
+            sumN -= dsum;
         }
     }
     // reduce (best, bidx) over the G threads of the pixel
@@ -261,19 +279,26 @@ cudaError_t launch_enumerate_n(const QaDevModel *d_model, QaWorkspace ws, QaCall
                                qa_stats *d_stats, cudaStream_t stream)
 {
     cudaError_t err;
+    const bool dep = args.closed && args.alg == QA_ALG_BRUTE_FORCE;  // closed brute force: the last dot follows from N_hat
+    if (dep) expect_cand /= (double)(args.n_max + 1);
+#define QA_ENUM_LAUNCH(GG, BLOCKS)                                                                                      \
+    (dep ? qa_launch_pdl(qa_enumerate_kernel<N, GG, true>, dim3(BLOCKS), dim3(ENUM_THREADS), stream, d_model, ws, args, \
+                         d_stats)                                                                                       \
+         : qa_launch_pdl(qa_enumerate_kernel<N, GG, false>, dim3(BLOCKS), dim3(ENUM_THREADS), stream, d_model, ws, args, \
+                         d_stats))
     if (expect_cand <= 64.0) {
         const unsigned blocks = (unsigned)((ws.P + ENUM_THREADS - 1) / ENUM_THREADS);
-        err = qa_launch_pdl(qa_enumerate_kernel<N, 1>, dim3(blocks), dim3(ENUM_THREADS), stream, d_model, ws, args, d_stats);
+        err = QA_ENUM_LAUNCH(1, blocks);
         qa_plan_add("qa_enumerate_kernel<G=1>");
     } else if (expect_cand <= 4096.0) {
         const unsigned blocks = (unsigned)((ws.P * 32 + ENUM_THREADS - 1) / ENUM_THREADS);
-        err = qa_launch_pdl(qa_enumerate_kernel<N, 32>, dim3(blocks), dim3(ENUM_THREADS), stream, d_model, ws, args, d_stats);
+        err = QA_ENUM_LAUNCH(32, blocks);
         qa_plan_add("qa_enumerate_kernel<G=32>");
     } else {
-        err = qa_launch_pdl(qa_enumerate_kernel<N, ENUM_THREADS>, dim3((unsigned)ws.P), dim3(ENUM_THREADS), stream, d_model, ws,
-                            args, d_stats);
+        err = QA_ENUM_LAUNCH(ENUM_THREADS, (unsigned)ws.P);
         qa_plan_add("qa_enumerate_kernel<G=256>");
     }
+#undef QA_ENUM_LAUNCH
     return err;
 }
 
