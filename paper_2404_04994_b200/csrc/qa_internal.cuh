@@ -141,36 +141,13 @@ __device__ __forceinline__ void qa_lexmin(double &e, uint64_t &i, double e2, uin
         i = i2;
     }
 }
-// S7 + S8 for one pixel, one thread: N* = base + digits of the winning mixed-radix index `idx`; E(N*) recomputed from the
-// definition (Eq. (C1) L607); sensor dots (L149 + Eq. (3) L41, reading R8).  idx = ~0: empty candidate set.
-__device__ __forceinline__ void qa_finalize_pixel(const QaDevModel *__restrict__ mdl, const double *__restrict__ Vg,
-                                                  const QaWorkspace &ws, int64_t p, uint64_t idx,
-                                                  int32_t *__restrict__ outN, double *__restrict__ outE,
-                                                  double *__restrict__ outVs)
+// S8 for one pixel: with the array charges Ns[0..n-1] fixed, every sensor dot's carrier number (lower energy of
+// max(0, floor s) and that + 1, s = N_c,s - M_sD d_D / M_ss) in the full model, the full charge row and the sensor
+// potentials V_s = [M (N - N_c)]_s (L149, Eq. (3), reading R8).
+__device__ __forceinline__ void qa_sensor_pixel(const QaDevModel *__restrict__ mdl, const double *__restrict__ Vg, int64_t p,
+                                                const int32_t *Ns, int32_t *__restrict__ outN, double *__restrict__ outVs)
 {
-    const int64_t P = ws.P;
     const int n = mdl->n, nf = mdl->nf, ns = mdl->ns, g = mdl->g;
-    int32_t Ns[QA_MAXN];
-    double d[QA_MAXN];
-    const bool empty = idx == ~0ull;
-    for (int i = n - 1; i >= 0; --i) {
-        const uint64_t c = (uint64_t)ws.cnt[i * P + p];
-        const int32_t dgt = (int32_t)(idx % c);
-        idx /= c;
-        Ns[i] = empty ? -1 : ws.base[i * P + p] + dgt;
-        d[i] = (double)Ns[i] - ws.nc[i * P + p];
-    }
-    double E = 0.0;
-    for (int i = 0; i < n; ++i) {
-        double row = 0.0;
-        for (int j = 0; j < n; ++j) row = fma(mdl->M[i * QA_MAXN + j], d[j], row);
-        E = fma(d[i], row, E);
-    }
-    outE[p] = empty ? INFINITY : 0.5 * E;
-    if (ns == 0) {
-        for (int i = 0; i < n; ++i) outN[p * n + i] = Ns[i];
-        return;
-    }
     // full model: N_c of every dot (same fma order), array dots fixed, then each sensor independently
     double ncf[QA_MAXN], df[QA_MAXN];
     int32_t Nf[QA_MAXN];
@@ -215,5 +192,38 @@ __device__ __forceinline__ void qa_finalize_pixel(const QaDevModel *__restrict__
             outVs[p * ns + a] = vsum;
         }
     }
+}
+
+// S7 + S8 for one pixel, one thread: N* = base + digits of the winning mixed-radix index `idx`; E(N*) recomputed from the
+// definition (Eq. (C1) L607); sensor dots (L149 + Eq. (3) L41, reading R8).  idx = ~0: empty candidate set.
+__device__ __forceinline__ void qa_finalize_pixel(const QaDevModel *__restrict__ mdl, const double *__restrict__ Vg,
+                                                  const QaWorkspace &ws, int64_t p, uint64_t idx,
+                                                  int32_t *__restrict__ outN, double *__restrict__ outE,
+                                                  double *__restrict__ outVs)
+{
+    const int64_t P = ws.P;
+    const int n = mdl->n, nf = mdl->nf, ns = mdl->ns, g = mdl->g;
+    int32_t Ns[QA_MAXN];
+    double d[QA_MAXN];
+    const bool empty = idx == ~0ull;
+    for (int i = n - 1; i >= 0; --i) {
+        const uint64_t c = (uint64_t)ws.cnt[i * P + p];
+        const int32_t dgt = (int32_t)(idx % c);
+        idx /= c;
+        Ns[i] = empty ? -1 : ws.base[i * P + p] + dgt;
+        d[i] = (double)Ns[i] - ws.nc[i * P + p];
+    }
+    double E = 0.0;
+    for (int i = 0; i < n; ++i) {
+        double row = 0.0;
+        for (int j = 0; j < n; ++j) row = fma(mdl->M[i * QA_MAXN + j], d[j], row);
+        E = fma(d[i], row, E);
+    }
+    outE[p] = empty ? INFINITY : 0.5 * E;
+    if (ns == 0) {
+        for (int i = 0; i < n; ++i) outN[p * n + i] = Ns[i];
+        return;
+    }
+    qa_sensor_pixel(mdl, Vg, p, Ns, outN, outVs);
 }
 #endif
