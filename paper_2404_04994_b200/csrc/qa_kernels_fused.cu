@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
                                                                     const double *__restrict__ Vg, int64_t P,
                                                                     QaCallArgs args, int32_t *__restrict__ outN,
                                                                     double *__restrict__ outE, double *__restrict__ xcont,
-                                                                    qa_stats *stats)
+                                                                    double *__restrict__ outVs, qa_stats *stats)
 {
     __shared__ double sM[N * N], sC[N * N], sCgd[N * QA_MAXG], sC1[N];
     __shared__ __align__(16) double sT[1 << N];  // pair table in Gray-walk order: sT[k] = QL[gray(k)]
@@ -204,8 +204,12 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
             Ed = fma(d[i], row, Ed);
         }
         outE[gp] = empty ? INFINITY : 0.5 * Ed;
+        if (mdl->ns == 0) {
 #pragma unroll
-        for (int i = 0; i < N; ++i) outN[gp * N + i] = Ns[i];
+            for (int i = 0; i < N; ++i) outN[gp * N + i] = Ns[i];
+        } else {  // S8: sensor dots in the full model (single-model calls only: gp = p)
+            qa_sensor_pixel(mdl, Vg, gp, Ns, outN, outVs);
+        }
         if (xcont) {
 #pragma unroll
             for (int i = 0; i < N; ++i) xcont[gp * N + i] = x[i];
@@ -225,27 +229,28 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
 
 template <int N>
 cudaError_t launch_fused_n(const QaDevModel *const *d_models, int n_models, const double *d_Vg, int64_t P, QaCallArgs args,
-                           int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats, cudaStream_t stream)
+                           int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs, qa_stats *d_stats, cudaStream_t stream)
 {
     const dim3 grid((unsigned)((P + FS_THREADS - 1) / FS_THREADS), (unsigned)n_models);
     if (args.alg == QA_ALG_DEFAULT && !args.closed)
-        qa_fused_small_kernel<N, true><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_stats);
+        qa_fused_small_kernel<N, true><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats);
     else
-        qa_fused_small_kernel<N, false><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_stats);
+        qa_fused_small_kernel<N, false><<<grid, FS_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats);
     return cudaGetLastError();
 }
 
 }  // namespace
 
 // d_models: device array of n_models device model pointers (all with the same n <= QA_FUSED_MAXN dots and g gates, no
-// sensor dots); V_g is [n_models][P][g], N is [n_models][P][n], E is [n_models][P].
+// sensor dots for n_models > 1); V_g is [n_models][P][g], N is [n_models][P][n], E is [n_models][P].  A single model with
+// sensor dots writes N as [P][n_full] and the sensor potentials d_Vs [P][n_sensor] (may be NULL).
 cudaError_t qa_launch_fused_small(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
-                                  QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats,
-                                  cudaStream_t stream)
+                                  QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
+                                  qa_stats *d_stats, cudaStream_t stream)
 {
     qa_plan_add("qa_fused_small_kernel");
     if (n_models > 65535) return cudaErrorInvalidValue;
-#define CALL(NN) launch_fused_n<NN>(d_models, n_models, d_Vg, P, args, d_N, d_E, d_xcont, d_stats, stream)
+#define CALL(NN) launch_fused_n<NN>(d_models, n_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats, stream)
     switch (n) {
         case 1: return CALL(1);
         case 2: return CALL(2);
