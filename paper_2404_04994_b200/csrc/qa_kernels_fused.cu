@@ -10,7 +10,8 @@
 // in lexicographic order (dot 0 most significant; strict '<' keeps the lexicographically first of equal energies, R6),
 // and E(N*) recomputed from the definition.  The open default set (every dot has exactly two values) is scored with the
 // static Gray walk of qa_kernels_walk.cu instead (3 FP64 instructions per candidate; pair table staged in shared memory).
-// Closed arrays score only candidates with sum N = N_hat (L127, L159).
+// Closed arrays score only candidates with sum N = N_hat (L127, L159).  A single model with charge-sensor dots (L149,
+// reading R8) also gets its sensor step S8 here (qa_sensor_pixel).
 #include "qa_internal.cuh"
 #include "qa_prologue.cuh"
 
