@@ -224,7 +224,8 @@ def run_ours(args, rank, world, local_rank):
     # beside the headline, never instead of it
     pruned = None
     if args.workload == "config4":
-        api.set_walk_variant(2)
+        for m_ in models:
+            m_.set_walk_variant(2)
         try:
             for _ in range(3):
                 step()
@@ -242,7 +243,8 @@ def run_ours(args, rank, world, local_rank):
                       "note": "qa_set_walk_variant(2): high patterns excluded by a rigorous lower bound are not walked; "
                               "identical N and E (tests/test_gpu_parity.py)"}
         finally:
-            api.set_walk_variant(1)
+            for m_ in models:
+                m_.set_walk_variant(1)
 
     # ---- per-kernel share of the step: CUDA events between the kernels (separate pass, same launch configuration) --
     kt = api.kernel_times(models[0], Vgs[0], steps=args.steps, flush=flush)

@@ -17,7 +17,8 @@
  *   - qa_ground_state_open / _closed are ASYNCHRONOUS on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream): they only enqueue kernels, never synchronise and never allocate.
  *   - A qa_model is immutable after qa_model_set_sensor_dots and may be used by concurrent calls on different streams
- *     (each call needs its own workspace).
+ *     (each call needs its own workspace).  It belongs to the CUDA device that was current at qa_model_create: every
+ *     call that takes the model (or a batch of models) returns QA_ERR_INVALID_ARG when another device is current.
  *   - Errors are returned as qa_status; nothing throws or aborts.  There is no CPU fallback: without a CUDA device every
  *     entry point that needs one returns QA_ERR_CUDA.
  */
@@ -65,10 +66,11 @@ typedef struct {
     int64_t n_qp_rounds;             /* total active-set rounds over those pixels                                      */
     int64_t n_candidates_enumerated; /* sum over pixels of the size of the enumerated set                              */
     int64_t n_candidates_scored;     /* ... of those whose energy entered the argmin (closed: sum N = N_hat); with the
-                                        pruned walk (qa_set_walk_variant(2)) it still counts the whole set: the pruned
-                                        candidates are covered by a bound                                              */
+                                        pruned walk (qa_model_set_walk_variant(m, 2)) it still counts the whole set:
+                                        the pruned candidates are covered by a bound                                   */
     int64_t n_threshold_doublings;   /* closed + thresholded: times t was doubled (L141, reading R5)                   */
-    int64_t n_widened_pixels;        /* closed: floor/ceil set empty even at t = 1, set widened (reading R5)           */
+    int64_t n_widened_pixels;        /* always 0 (kept for layout): the closed floor/ceil set is never empty at t = 1, so
+                                        the widened set of an earlier reading R5 does not exist (R5)         */
     int64_t n_qp_failed;             /* pixels whose QP did not reach a KKT point (must be 0)                          */
 } qa_stats;
 
@@ -171,30 +173,9 @@ QA_API qa_status qa_ground_state_batch(const qa_batch *batch, const double *d_Vg
                                        qa_algorithm alg, double t, int n_max, int32_t *d_N, double *d_E, double *d_xcont,
                                        qa_stats *d_stats, void *cuda_stream);
 
-/* ---- measurement aids -------------------------------------------------------------------------------------------- */
-
-/* Sustained FP64 issue rate of the current device: independent DFMA chains on every SM for about `seconds`.
- * Returns FP64 thread-instructions per second (1 DFMA = 1) -- the denominator of the ALU roofline. */
-QA_API qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *cuda_stream);
-
-/* Per-kernel timing of a call (measurement aid, per host thread).  While enabled, qa_ground_state_open / _closed record
- * CUDA events on the call's stream before the first and after every kernel.  qa_get_kernel_timings waits for the last
- * event of the most recent call and returns the device time of each of its kernels in milliseconds, in launch order
- * (names: qa_last_launch_plan).  ms: host, max_kernels floats; *n_kernels: how many were written. */
-QA_API qa_status qa_set_kernel_timing(int enable);
-QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernels);
-
-/* Kernel selection (process-wide; cross-check aid, the results are identical): 0 = the three-kernel path for every n_dot
- * (prologue, exact-compare Gray walk or enumeration, finalize), 1 (default) = the min-plus walk with its finish kernel for
- * the open default search of n_dot >= 13 and the one-kernel path for n_dot <= 8, 2 = as 1, but the
- * open default search of n_dot >= 13 skips the high patterns a rigorous lower bound excludes (same arg min; fewer
- * candidates are scored explicitly).  Returns QA_ERR_INVALID_ARG for any other value. */
-QA_API qa_status qa_set_walk_variant(int variant);
-
-/* Names of the kernels the last ground-state call on this host thread enqueued (comma separated; static storage). */
-QA_API const char *qa_last_launch_plan(void);
-/* Number of kernels the last ground-state call on this host thread enqueued. */
-QA_API int qa_last_launch_count(void);
+/* ---- diagnostics ------------------------------------------------------------------------------------------------- */
+/* (Measurement and cross-check aids -- FP64 issue-rate probe, per-kernel event timing, launch plan, kernel selection --
+ * are declared in qarray_b200_aids.h; they are not part of the product surface.) */
 
 QA_API const char *qa_status_string(qa_status s);
 QA_API const char *qa_last_cuda_error(void);

@@ -38,7 +38,7 @@ def _lib(omp: bool = False):
         lib.qo_thermal.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp,
                                    lp, ip]
         lib.qo_sensor.argtypes = [vp, vp, ip, C.c_int, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip,
-                                  dp, dp, dp, ip]
+                                  dp, dp, dp, dp, ip]
         _libs[key] = lib
     return _libs[key]
 
@@ -160,7 +160,8 @@ Model.thermal = _thermal
 
 
 def sensor_ground_state(C_dd, C_gd, sensor_dots, Vg, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0):
-    """Reading R8: array sub-problem on the sub-blocks, then the sensor dots.  Returns dict(N[P,n_full], E, E2, Vs[P,ns], flags)."""
+    """Reading R8: array sub-problem on the sub-blocks, then the sensor dots.  Returns dict(N[P,n_full], E, E2, Vs[P,ns],
+    sgap[P,ns] = margin |e(c0+1) - e(c0)| of every sensor's two-way choice, flags)."""
     C_dd = np.ascontiguousarray(C_dd, dtype=np.float64)
     C_gd = np.ascontiguousarray(C_gd, dtype=np.float64)
     n = C_dd.shape[0]
@@ -171,10 +172,10 @@ def sensor_ground_state(C_dd, C_gd, sensor_dots, Vg, regime="open", N_hat=0, alg
     Vg = np.ascontiguousarray(Vg, dtype=np.float64).reshape(-1, full.g)
     P = Vg.shape[0]
     out = dict(N=np.empty((P, n), np.int32), E=np.empty(P), E2=np.empty(P), Vs=np.empty((P, len(sens))),
-               flags=np.empty(P, np.int32))
+               sgap=np.empty((P, len(sens))), flags=np.empty(P, np.int32))
     rc = _lib().qo_sensor(full._buf, sub._buf, _ip(sens), len(sens), _dp(Vg), P, int(regime == "closed"), int(N_hat),
                           ALG[algorithm], float(t), int(n_max), _ip(out["N"]), _dp(out["E"]), _dp(out["E2"]),
-                          _dp(out["Vs"]), _ip(out["flags"]))
+                          _dp(out["Vs"]), _dp(out["sgap"]), _ip(out["flags"]))
     if rc:
         raise ValueError(f"qo_sensor: invalid argument ({rc})")
     return out

@@ -42,7 +42,7 @@
 #define QO_ALG_BRUTE 2
 
 #define QO_FLAG_QP 1        /* analytic minimum had a negative component; QP solved        */
-#define QO_FLAG_WIDENED 2   /* closed: floor/ceil set empty even at t = 1; widened (R5)    */
+#define QO_FLAG_WIDENED 2   /* never set: the widened set of an earlier reading R5 is unreachable (R5) */
 #define QO_FLAG_QP_FAIL 4   /* KKT certificate not met / iteration cap (must never happen) */
 #define QO_FLAG_EMPTY 8     /* no admissible candidate (closed brute force with n*n_max < N_hat) */
 
@@ -436,15 +436,9 @@ int qo_pixel(const qo_model *m, const double *Vg, int closed, int N_hat, int alg
                 doublings++;
                 ranges_floor_ceil(n, x, tt, 1, base, cnt);
             }
-            if (!closed_nonempty(n, base, cnt, N_hat)) { /* R5 fallback, expected never */
-                flags |= QO_FLAG_WIDENED;
-                for (int i = 0; i < n; i++) {
-                    double fl = floor(x[i]);
-                    int32_t lo = fl > 0.0 ? (int32_t)fl : 0;
-                    base[i] = lo > 0 ? lo - 1 : 0;
-                    cnt[i] = lo + 2 - base[i] + 1;
-                }
-            }
+            /* At t = 1 the kept set is the closed default set, which is never empty for a feasible x (x >= 0,
+             * |sum x - N_hat| << 1): sum lo <= sum x and sum (lo + 1) > sum x, so 0 <= N_hat - sum lo <= n
+             * (reading R5).  Should it ever be empty the pixel is reported as QO_FLAG_EMPTY below. */
         }
     }
     qo_best b;
@@ -500,14 +494,6 @@ int qo_pixel_thermal(const qo_model *m, const double *Vg, int closed, int N_hat,
             while (alg == QO_ALG_THRESHOLDED && !closed_nonempty(n, base, cnt, N_hat) && tt < 1.0) {
                 tt = (tt > 0.0) ? fmin(1.0, 2.0 * tt) : 1.0;
                 ranges_floor_ceil(n, x, tt, 1, base, cnt);
-            }
-            if (!closed_nonempty(n, base, cnt, N_hat)) {
-                for (int i = 0; i < n; i++) {
-                    double fl = floor(x[i]);
-                    int32_t lo = fl > 0.0 ? (int32_t)fl : 0;
-                    base[i] = lo > 0 ? lo - 1 : 0;
-                    cnt[i] = lo + 2 - base[i] + 1;
-                }
             }
         }
     }
@@ -596,9 +582,11 @@ int qo_ground_state(const qo_model *m, const double *Vg, int64_t P, int closed, 
 /*        y = sum_{j in D} M_sj (N_j - N_c,j);  s* = N_c,s - y / M_ss;  c0 = max(0, floor s*);                          */
 /*        e(c) = (c - N_c,s) y + 1/2 M_ss (c - N_c,s)^2;   N_s = c0 + 1 if e(c0 + 1) < e(c0) else c0                   */
 /*   c. V_s = [M (N - N_c)]_s over the full model with every N_s set  (Eq. (3) with the positive-C_gd convention)      */
+/* sgap (optional) returns |e(c0 + 1) - e(c0)| per sensor: the margin of step b's two-way choice, so that the parity   */
+/* tests can apply the near-tie rule (margin < 1e-9 E_C) to the sensor columns as they do to the array columns.        */
 int qo_sensor(const qo_model *full, const qo_model *sub, const int32_t *sensor_idx, int ns, const double *Vg, int64_t P,
               int closed, int N_hat, int alg, double t, int n_max, int32_t *N /* [P][n_full] */, double *E /* [P] */,
-              double *E2, double *Vs /* [P][ns] */, int32_t *flags)
+              double *E2, double *Vs /* [P][ns] */, double *sgap /* [P][ns] |e(c0+1) - e(c0)| or NULL */, int32_t *flags)
 {
     int n = full->n, g = full->g;
     if (sub->n != n - ns || sub->g != g || ns < 1 || ns >= n) return 1;
@@ -636,6 +624,7 @@ int qo_sensor(const qo_model *full, const qo_model *sub, const int32_t *sensor_i
             double e0 = d0 * y + 0.5 * Mss * d0 * d0;
             double e1 = d1 * y + 0.5 * Mss * d1 * d1;
             Np[s] = (e1 < e0) ? c0 + 1 : c0;
+            if (sgap) sgap[p * ns + a] = fabs(e1 - e0); /* the two-way choice's margin (near-tie rule of the parity tests) */
         }
         for (int a = 0; a < ns; a++) d[sensor_idx[a]] = (double)Np[sensor_idx[a]] - Nc[sensor_idx[a]];
         for (int a = 0; a < ns; a++) {

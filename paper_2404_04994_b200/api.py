@@ -23,7 +23,7 @@ STATUS_NAMES = ["QA_OK", "QA_ERR_INVALID_ARG", "QA_ERR_NOT_SYMMETRIC", "QA_ERR_N
 EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "qa_model_n_dot", "qa_model_n_gate",
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
            "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
-           "qa_get_kernel_timings", "qa_set_walk_variant", "qa_batch_create", "qa_batch_destroy", "qa_batch_size",
+           "qa_get_kernel_timings", "qa_model_set_walk_variant", "qa_batch_create", "qa_batch_destroy", "qa_batch_size",
            "qa_ground_state_batch", "qa_thermal_open", "qa_thermal_closed", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
 
@@ -81,7 +81,7 @@ def lib() -> C.CDLL:
                                         C.c_size_t, vp]
         l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
         l.qa_set_kernel_timing.argtypes = [C.c_int]
-        l.qa_set_walk_variant.argtypes = [C.c_int]
+        l.qa_model_set_walk_variant.argtypes = [vp, C.c_int]
         l.qa_get_kernel_timings.argtypes = [C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_int)]
         l.qa_last_launch_plan.restype = C.c_char_p
         l.qa_status_string.restype = C.c_char_p
@@ -104,7 +104,7 @@ def _ptr(t):
 class Model:
     """qa_model_create(C_dd, C_gd).  Owns the opaque handle."""
 
-    def __init__(self, C_dd, C_gd, sensor_dots=()):
+    def __init__(self, C_dd, C_gd, sensor_dots=(), walk_variant=None):
         C_dd = np.ascontiguousarray(C_dd, dtype=np.float64)
         C_gd = np.ascontiguousarray(C_gd, dtype=np.float64)
         if C_dd.ndim != 2 or C_dd.shape[0] != C_dd.shape[1] or C_gd.ndim != 2 or C_gd.shape[0] != C_dd.shape[0]:
@@ -112,10 +112,22 @@ class Model:
         self._h = C.c_void_p()
         _check(lib().qa_model_create(C_dd.ctypes.data, C_gd.ctypes.data, C_dd.shape[0], C_gd.shape[1],
                                      C.byref(self._h)), "qa_model_create")
+        self.device = torch.device("cuda", torch.cuda.current_device()) if torch.cuda.is_available() else None
         if len(sensor_dots):
             self.set_sensor_dots(sensor_dots)
+        if walk_variant is not None:
+            self.set_walk_variant(walk_variant)
         self._ws = None
         self._stats = None
+
+    def set_walk_variant(self, variant: int):
+        """qa_model_set_walk_variant (cross-check aid, qarray_b200_aids.h): 0 = three-kernel path with the exact-compare walk /
+        generic enumeration everywhere, 1 = production dispatch, 2 = as 1 with exact pruning in the 13..16-dot min-plus walk."""
+        _check(lib().qa_model_set_walk_variant(self._h, int(variant)), "qa_model_set_walk_variant")
+
+    def _check_device(self, Vg):
+        if Vg.device != self.device:
+            raise ValueError(f"Vg is on {Vg.device}, the model lives on {self.device}")
 
     def set_sensor_dots(self, dots):
         idx = np.ascontiguousarray(dots, dtype=np.int32)
@@ -159,6 +171,7 @@ class Model:
         current torch stream.  Returns dict(N, E[, xcont][, Vsensor][, stats (a device tensor of 8 int64)])."""
         if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
             raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        self._check_device(Vg)
         Vg = Vg.contiguous().view(-1, self.n_gate)
         P, dev = Vg.shape[0], Vg.device
         out = out or {}
@@ -177,14 +190,11 @@ class Model:
         s = stream if stream is not None else torch.cuda.current_stream(dev)
         sp = C.c_void_p(s.cuda_stream)
         alg = ALG[algorithm] if isinstance(algorithm, str) else int(algorithm)
-        if regime == "open":
-            rc = lib().qa_ground_state_open(self._h, _ptr(Vg), P, alg, float(t), int(n_max), _ptr(N), _ptr(E), _ptr(xc),
-                                            _ptr(Vs), _ptr(st), _ptr(ws), ws.numel(), sp)
-        elif regime == "closed":
-            rc = lib().qa_ground_state_closed(self._h, _ptr(Vg), P, int(N_hat), alg, float(t), int(n_max), _ptr(N),
-                                              _ptr(E), _ptr(xc), _ptr(Vs), _ptr(st), _ptr(ws), ws.numel(), sp)
+        if torch.cuda.current_device() != dev.index:      # the C call checks the current device against the model's
+            with torch.cuda.device(dev):
+                rc = self._call_ground_state(regime, Vg, P, N_hat, alg, t, n_max, N, E, xc, Vs, st, ws, sp)
         else:
-            raise ValueError("regime must be 'open' or 'closed'")
+            rc = self._call_ground_state(regime, Vg, P, N_hat, alg, t, n_max, N, E, xc, Vs, st, ws, sp)
         _check(rc, f"qa_ground_state_{regime}")
         res = {"N": N, "E": E}
         if xc is not None:
@@ -195,12 +205,24 @@ class Model:
             res["stats"] = st
         return res
 
+    def _call_ground_state(self, regime, Vg, P, N_hat, alg, t, n_max, N, E, xc, Vs, st, ws, sp):
+        if regime == "open":
+            rc = lib().qa_ground_state_open(self._h, _ptr(Vg), P, alg, float(t), int(n_max), _ptr(N), _ptr(E), _ptr(xc),
+                                            _ptr(Vs), _ptr(st), _ptr(ws), ws.numel(), sp)
+        elif regime == "closed":
+            rc = lib().qa_ground_state_closed(self._h, _ptr(Vg), P, int(N_hat), alg, float(t), int(n_max), _ptr(N),
+                                              _ptr(E), _ptr(xc), _ptr(Vs), _ptr(st), _ptr(ws), ws.numel(), sp)
+        else:
+            raise ValueError("regime must be 'open' or 'closed'")
+        return rc
+
     def thermal(self, Vg: torch.Tensor, kT: float, regime="open", N_hat=0, algorithm="default", t=1.0, n_max=0,
                 want_stats=False, stream=None):
         """qa_thermal_open / qa_thermal_closed: Eq. (10) mean occupation on a CUDA tensor Vg[P, n_gate].  Returns
         dict(Nmean[P, n_search] float64, Emin[P][, stats])."""
         if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
             raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        self._check_device(Vg)
         Vg = Vg.contiguous().view(-1, self.n_gate)
         P, dev = Vg.shape[0], Vg.device
         Nm = torch.empty((P, self.n_search), dtype=torch.float64, device=dev)
@@ -263,6 +285,7 @@ class Batch:
         self._h = C.c_void_p()
         _check(lib().qa_batch_create(arr, len(self.models), C.byref(self._h)), "qa_batch_create")
         self.n_dot, self.n_gate = self.models[0].n_dot, self.models[0].n_gate
+        self.device = self.models[0].device
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -283,6 +306,8 @@ class Batch:
         """qa_ground_state_batch on a CUDA tensor Vg[B, P, n_gate] (float64).  Returns dict(N[B,P,n], E[B,P], ...)."""
         if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
             raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        if Vg.device != self.device:
+            raise ValueError(f"Vg is on {Vg.device}, the batch lives on {self.device}")
         B = len(self)
         Vg = Vg.contiguous().view(B, -1, self.n_gate)
         P, dev = Vg.shape[1], Vg.device
@@ -337,12 +362,6 @@ def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch
     finally:
         lib().qa_set_kernel_timing(0)
     return acc
-
-
-def set_walk_variant(variant: int) -> None:
-    """qa_set_walk_variant: 0 = three-kernel path everywhere, 1 = default (min-plus walk for n_dot >= 13, one-kernel path
-    for n_dot <= 8), 2 = as 1 with exact pruning of the high patterns in the min-plus walk."""
-    _check(lib().qa_set_walk_variant(int(variant)), "qa_set_walk_variant")
 
 
 def last_launch_plan():

@@ -1,5 +1,6 @@
 // qa_api.cu -- host side of the C ABI (include/qarray_b200.h): model validation and setup (S0), argument checks,
 // workspace carving and kernel dispatch.  No compute on the host beyond S0; no CPU fallback.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -9,11 +10,13 @@
 #include <string>
 
 #include "qa_internal.cuh"
+#include "../../include/qarray_b200_aids.h"
 
 struct qa_batch {
     int n_models, n, g, general;
     int device;
     const QaDevModel **dev_list;  // device array of the models' device pointers
+    qa_model **members;           // host: the models (their in_batches count is held until qa_batch_destroy)
 };
 
 struct qa_model {
@@ -30,6 +33,8 @@ struct qa_model {
     QaDevModel *dev;        // device copy
     const QaDevModel **dev_self;  // device array of one pointer (= dev): the model list of a single-model fused launch
     QaWalkTable walk;       // pair table of the low bits of the search model
+    std::atomic<int> walk_variant;  // kernel selection (qa_model_set_walk_variant; cross-check aid)
+    std::atomic<int> in_batches;    // qa_batch objects holding this model's device pointer
     // qa_ground_state_host: a private stream and a grow-only device staging buffer, reused from call to call (creating
     // a stream and going through the allocator cost more than the search itself on a 100x100 diagram)
     std::mutex host_mu;
@@ -169,23 +174,26 @@ qa_status rebuild(qa_model *m)
             h.QHT[t] = q;
         }
     }
+    // The source is pageable and the kernels run on non-blocking streams, which are not ordered against the legacy
+    // stream: wait until the copy has landed and nothing else on the device can still read the old constants.
     QA_CUDA(cudaMemcpy(m->dev, &h, sizeof(h), cudaMemcpyHostToDevice));
+    QA_CUDA(cudaDeviceSynchronize());
     return QA_OK;
 }
 
-// qa_set_walk_variant (cross-check aid): which kernel scores the open/default candidates of arrays with n >= 13.
-// 0 = the three-kernel path everywhere (prologue, exact-compare Gray walk or enumeration, finalize), 1 (default) = the
-// min-plus walk + finish kernel for n >= 13 and the one-kernel path for n <= 8.  Initial value from the
-// environment variable QA_WALK_VARIANT.
-int g_walk_variant = -1;
-int walk_variant()
+// Initial kernel selection of a model (qa_model_set_walk_variant): environment variable QA_WALK_VARIANT, default 1.
+int initial_walk_variant()
 {
-    if (g_walk_variant < 0) {
-        const char *e = std::getenv("QA_WALK_VARIANT");
-        g_walk_variant = e ? std::atoi(e) : 1;
-        if (g_walk_variant < 0 || g_walk_variant > 2) g_walk_variant = 1;
-    }
-    return g_walk_variant;
+    const char *e = std::getenv("QA_WALK_VARIANT");
+    const int v = e ? std::atoi(e) : 1;
+    return (v < 0 || v > 2) ? 1 : v;
+}
+
+// A model (batch) belongs to the device that was current when it was created.
+bool on_device(int device)
+{
+    int cur = -1;
+    return cudaGetDevice(&cur) == cudaSuccess && cur == device;
 }
 
 size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
@@ -230,6 +238,8 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
 {
     qa_plan_reset();
     if (!m || P < 0 || (P > 0 && (!d_Vg || !d_N || !d_E))) return QA_ERR_INVALID_ARG;
+    if (P > 0 && !on_device(m->device)) return QA_ERR_INVALID_ARG;
+    const int variant = m->walk_variant.load(std::memory_order_relaxed);
     if (alg != QA_ALG_DEFAULT && alg != QA_ALG_THRESHOLDED && alg != QA_ALG_BRUTE_FORCE) return QA_ERR_INVALID_ARG;
     if (alg == QA_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return QA_ERR_INVALID_ARG;
     if (alg == QA_ALG_BRUTE_FORCE && n_max < 0) return QA_ERR_INVALID_ARG;
@@ -252,7 +262,7 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     // small arrays with small candidate sets: the whole path in one kernel, one thread per pixel (no workspace traffic)
     {
         const double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n) : std::pow(2.0, (double)n);
-        if (n <= QA_FUSED_MAXN && expect <= 256.0 && walk_variant() != 0) {
+        if (n <= QA_FUSED_MAXN && expect <= 256.0 && variant != 0) {
             QA_CUDA(qa_launch_fused_small(m->dev_self, 1, n, d_Vg, P, a, d_N, d_E, d_xcont, m->ns > 0 ? d_Vsensor : nullptr,
                                           d_stats, stream));
             timing_mark(stream);
@@ -262,10 +272,10 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
     timing_mark(stream);
     // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd
-    if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && walk_variant() != 0 && m->is_z) {
+    if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && variant != 0 && m->is_z) {
         const bool fuse = m->ns == 0;  // S7 runs inside the finish kernel: no finalize launch
         QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count,
-                                       walk_variant() == 2, stream));
+                                       variant == 2, stream));
         timing_mark(stream);
         if (fuse) return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && !closed) {
@@ -290,6 +300,7 @@ qa_status thermal(const qa_model *m, const double *d_Vg, int64_t P, int closed, 
 {
     qa_plan_reset();
     if (!m || P < 0 || (P > 0 && (!d_Vg || !d_Nmean))) return QA_ERR_INVALID_ARG;
+    if (P > 0 && !on_device(m->device)) return QA_ERR_INVALID_ARG;
     if (!(kT > 0.0) || !std::isfinite(kT)) return QA_ERR_INVALID_ARG;
     if (alg != QA_ALG_DEFAULT && alg != QA_ALG_THRESHOLDED && alg != QA_ALG_BRUTE_FORCE) return QA_ERR_INVALID_ARG;
     if (alg == QA_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return QA_ERR_INVALID_ARG;
@@ -361,6 +372,8 @@ qa_status qa_model_create(const double *C_dd, const double *C_gd, int n_dot, int
     m->g = n_gate;
     m->ns = 0;
     m->is_z = is_z;
+    m->walk_variant.store(initial_walk_variant());
+    m->in_batches.store(0);
     std::memcpy(m->Cf, C_dd, sizeof(double) * n_dot * n_dot);
     std::memcpy(m->Cgdf, C_gd, sizeof(double) * n_dot * n_gate);
     if (!spd_inverse(m->Cf, n_dot, m->Mf)) {
@@ -395,6 +408,7 @@ qa_status qa_model_create(const double *C_dd, const double *C_gd, int n_dot, int
 qa_status qa_model_set_sensor_dots(qa_model *m, const int *dot_idx, int n_sensor)
 {
     if (!m || n_sensor < 0 || n_sensor >= m->nf || (n_sensor > 0 && !dot_idx)) return QA_ERR_INVALID_ARG;
+    if (m->in_batches.load() != 0 || !on_device(m->device)) return QA_ERR_INVALID_ARG;  // a batch holds the old constants
     bool seen[QA_MAXN] = {false};
     for (int a = 0; a < n_sensor; ++a) {
         if (dot_idx[a] < 0 || dot_idx[a] >= m->nf || seen[dot_idx[a]]) return QA_ERR_INVALID_ARG;
@@ -465,6 +479,7 @@ qa_status qa_ground_state_host(const qa_model *mc, const double *h_Vg, int64_t P
 {
     if (!mc || P < 0 || (P > 0 && (!h_Vg || !h_N || !h_E))) return QA_ERR_INVALID_ARG;
     if (P == 0) return QA_OK;
+    if (!on_device(mc->device)) return QA_ERR_INVALID_ARG;
     qa_model *m = const_cast<qa_model *>(mc);  // only the host-call staging state below is touched, under its mutex
     std::lock_guard<std::mutex> lock(m->host_mu);
     const size_t Pz = (size_t)P, nf = (size_t)m->nf, n = (size_t)m->host.n, g = (size_t)m->g, ns = (size_t)m->ns;
@@ -548,18 +563,28 @@ qa_status qa_batch_create(const qa_model *const *models, int n_models, qa_batch 
         delete bt;
         return QA_ERR_INVALID_ARG;
     }
+    bt->members = new (std::nothrow) qa_model *[n_models];
+    if (!bt->members) {
+        delete[] list;
+        delete bt;
+        return QA_ERR_INVALID_ARG;
+    }
     for (int b = 0; b < n_models; ++b) {
         list[b] = models[b]->dev;
+        bt->members[b] = const_cast<qa_model *>(models[b]);
         if (!models[b]->is_z) bt->general = 1;
     }
     cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&bt->dev_list), sizeof(QaDevModel *) * n_models);
     if (e == cudaSuccess) e = cudaMemcpy(bt->dev_list, list, sizeof(QaDevModel *) * n_models, cudaMemcpyHostToDevice);
     delete[] list;
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();  // pageable source, non-blocking consumer streams (as in rebuild)
     if (e != cudaSuccess) {
         if (bt->dev_list) cudaFree(bt->dev_list);
+        delete[] bt->members;
         delete bt;
         return cuda_fail(e, "qa_batch_create");
     }
+    for (int b = 0; b < n_models; ++b) bt->members[b]->in_batches.fetch_add(1);
     *out = bt;
     return QA_OK;
 }
@@ -568,6 +593,8 @@ qa_status qa_batch_destroy(qa_batch *bt)
 {
     if (!bt) return QA_OK;
     cudaError_t e = cudaFree(bt->dev_list);
+    for (int b = 0; b < bt->n_models; ++b) bt->members[b]->in_batches.fetch_sub(1);
+    delete[] bt->members;
     delete bt;
     return e == cudaSuccess ? QA_OK : cuda_fail(e, "qa_batch_destroy");
 }
@@ -578,6 +605,7 @@ qa_status qa_ground_state_batch(const qa_batch *bt, const double *d_Vg, int64_t 
 {
     qa_plan_reset();
     if (!bt || P < 0 || (P > 0 && (!d_Vg || !d_N || !d_E))) return QA_ERR_INVALID_ARG;
+    if (P > 0 && !on_device(bt->device)) return QA_ERR_INVALID_ARG;
     if (alg != QA_ALG_DEFAULT && alg != QA_ALG_THRESHOLDED && alg != QA_ALG_BRUTE_FORCE) return QA_ERR_INVALID_ARG;
     if (alg == QA_ALG_THRESHOLDED && !(t >= 0.0 && t <= 1.0)) return QA_ERR_INVALID_ARG;
     if (alg == QA_ALG_BRUTE_FORCE && n_max < 0) return QA_ERR_INVALID_ARG;
@@ -643,10 +671,10 @@ qa_status qa_set_kernel_timing(int enable)
     return QA_OK;
 }
 
-qa_status qa_set_walk_variant(int variant)
+qa_status qa_model_set_walk_variant(qa_model *m, int variant)
 {
-    if (variant < 0 || variant > 2) return QA_ERR_INVALID_ARG;
-    g_walk_variant = variant;
+    if (!m || variant < 0 || variant > 2) return QA_ERR_INVALID_ARG;
+    m->walk_variant.store(variant, std::memory_order_relaxed);
     return QA_OK;
 }
 

@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
                                                                     double *__restrict__ outVs, qa_stats *stats)
 {
     __shared__ double sM[N * N], sC[N * N], sCgd[N * QA_MAXG], sC1[N];
-    __shared__ __align__(16) double sT[1 << N];  // pair table in Gray-walk order: sT[k] = QL[gray(k)]
+    __shared__ __align__(16) double sT[1 << N];  // pair table of the low-bit patterns: sT[k] = QL[k]
     const QaDevModel *__restrict__ mdl = models[blockIdx.y];
     const int g = mdl->g;
     for (int e = threadIdx.x; e < N * N; e += FS_THREADS) {
@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
     }
     for (int e = threadIdx.x; e < N * g; e += FS_THREADS) sCgd[e] = mdl->Cgd[(e / g) * QA_MAXG + (e % g)];
     if (threadIdx.x < N) sC1[threadIdx.x] = mdl->C1[threadIdx.x];
-    for (int k = threadIdx.x; k < (1 << N); k += FS_THREADS) sT[k] = mdl->QL[k ^ (k >> 1)];
+    for (int k = threadIdx.x; k < (1 << N); k += FS_THREADS) sT[k] = mdl->QL[k];
     const double oneC1 = mdl->oneC1;
     __syncthreads();
 
@@ -92,20 +92,26 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
         double hp[N];
 #pragma unroll
         for (int j = 0; j < N; ++j) hp[j] = grad[N - 1 - j] + 0.5 * sM[(N - 1 - j) * N + (N - 1 - j)];
+        // counting order (qa_kernels_walk.cu): step k-1 -> k moves the linear part by c_ctz(k); ascending k + strict '<'
+        // keeps the smallest index among bitwise-equal energies (reading R6)
+        double cj[N];
+        {
+            double pre = 0.0;
+#pragma unroll
+            for (int j = 0; j < N; ++j) {
+                cj[j] = hp[j] - pre;
+                pre += hp[j];
+            }
+        }
         double s = 0.0, m = 0.0;
         unsigned idx = 0;
 #pragma unroll
         for (int k = 1; k < (1 << N); ++k) {
-            const int j = fs_ctz(k);
-            const int gk = k ^ (k >> 1);
-            if ((gk >> j) & 1)
-                s += hp[j];
-            else
-                s -= hp[j];
+            s += cj[fs_ctz(k)];
             const double e = s + sT[k];
             if (e < m) {
                 m = e;
-                idx = gk;
+                idx = k;
             }
         }
         bidx = idx;
@@ -222,7 +228,6 @@ __global__ void __launch_bounds__(FS_THREADS, GRAY ? 2 : 4) qa_fused_small_kerne
         qa_warp_count(&stats->n_qp_rounds, live ? fl.rounds : 0);
         qa_warp_count(&stats->n_qp_failed, (live && fl.failed) ? 1 : 0);
         qa_warp_count(&stats->n_threshold_doublings, live ? fl.doublings : 0);
-        qa_warp_count(&stats->n_widened_pixels, (live && fl.widened) ? 1 : 0);
         qa_warp_count(&stats->n_candidates_enumerated, live ? (int64_t)total : 0);
         qa_warp_count(&stats->n_candidates_scored, live ? scored : 0);
     }

@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
     int32_t base[N], cnt[N];
     QaPixelFlags fl;
     qa_prologue_pixel<N>(sCgd, sC, sC1, oneC1, g, Vg + pp * g, args, nc, x, base, cnt, fl);
-    const bool neg = fl.neg, failed = fl.failed, widened = fl.widened;
+    const bool neg = fl.neg, failed = fl.failed;
     const int rounds = fl.rounds, doublings = fl.doublings;
     // base-point gradient
     double d0[N];
@@ -81,7 +81,6 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
         qa_warp_count(&stats->n_qp_rounds, live ? rounds : 0);
         qa_warp_count(&stats->n_qp_failed, (live && failed) ? 1 : 0);
         qa_warp_count(&stats->n_threshold_doublings, live ? doublings : 0);
-        qa_warp_count(&stats->n_widened_pixels, (live && widened) ? 1 : 0);
         qa_warp_count(&stats->n_candidates_enumerated, live ? (int64_t)total : 0);
         qa_warp_count(&stats->n_candidates_scored, (live && !closed) ? (int64_t)total : 0);  // open: all are scored
     }

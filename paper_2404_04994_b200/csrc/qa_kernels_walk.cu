@@ -5,14 +5,15 @@
 // so the pixel enters only through the n numbers h_i (written by the prologue); the pair term is pixel-independent.
 //
 // Decomposition (B200: FP64 pipe bound, 64 lanes/SM): the n bits are split into NH high bits, one thread per high
-// pattern t (2^NH threads share a pixel), and NL <= 8 low bits walked by each thread in binary-reflected Gray order,
-// fully unrolled so that every index is static:
+// pattern t (2^NH threads share a pixel), and NL <= 8 low bits walked by each thread in counting order (each step moves
+// the linear part by a per-pixel constant c_ctz(k), like a Gray step, and ascending order makes the tie-break of
+// reading R6 free), fully unrolled so that every index is static:
 //     per thread, once:   v_j  = sum_{hi bit j' in t} M[a_j][a_j']          (cross term hi x lo, pixel-independent)
 //                         QH   = sum_{hi pairs in t} M                      (pixel-independent)
 //     per thread x pixel: h'_j = h[a_j] + v_j   (NL adds),   base_t = QH + sum_{hi bits in t} h   (<= NH adds)
-//     per candidate:      s +-= h'_ctz(k)                       1 DADD   (running linear part, Gray step k)
-//                         e  = s + QL[gray(k)]                  1 DADD   (pair table of the low bits, constant bank)
-//                         (e < m) ? (m, idx) = (e, gray(k))     1 DSETP + selects
+//     per candidate:      s += c_ctz(k), c_j = h'_j - sum_{i<j} h'_i   1 DADD   (running linear part of pattern k)
+//                         e  = s + QL[k]                        1 DADD   (pair table of the low bits, constant bank)
+//                         (e < m) ? (m, idx) = (e, k)           1 DSETP + selects
 // i.e. 3 FP64-pipe instructions per candidate, independent of n (the definition costs n^2 + n FMAs, the lazy Gray update
 // of SURVEY.md section 8(d) about 5.5).  The winner over the 2^NH threads is taken by a lexicographic (E, index) min over
 // shuffles / shared memory, so the result does not depend on scheduling.  E(N*) itself is recomputed from the definition
@@ -81,21 +82,28 @@ __global__ void __launch_bounds__(WALK_THREADS) qa_walk_kernel(const QaDevModel 
         for (int jh = 0; jh < NH; ++jh)
             if ((t >> jh) & 1u) baseE += ws.h[(int64_t)(N - 1 - NL - jh) * P + pp];
 
-        // Gray walk over the 2^NL low patterns; k = 0 is the all-zero pattern with e = 0
+        // Walk over the 2^NL low patterns in counting order k = 0, 1, 2, ...: the step k-1 -> k sets bit j = ctz(k) and clears
+        // the bits below it, so the linear part moves by c_j = h'_j - sum_{i<j} h'_i whatever k is (one DADD, like a Gray
+        // step), and because k ascends the strict '<' keeps the smallest index among bitwise-equal energies (reading R6).
+        // k = 0 is the all-zero pattern with e = 0.
+        double cj[NL];
+        {
+            double pre = 0.0;
+#pragma unroll
+            for (int j = 0; j < NL; ++j) {
+                cj[j] = hp[j] - pre;
+                pre += hp[j];
+            }
+        }
         double s = 0.0, m = 0.0;
         unsigned idx = 0;
 #pragma unroll
         for (int k = 1; k < (1 << NL); ++k) {
-            const int j = qa_ctz(k);
-            const int gk = k ^ (k >> 1);
-            if ((gk >> j) & 1)
-                s += hp[j];
-            else
-                s -= hp[j];
-            const double e = s + tab.QL[gk];
+            s += cj[qa_ctz(k)];
+            const double e = s + tab.QL[k];
             if (e < m) {
                 m = e;
-                idx = gk;
+                idx = k;
             }
         }
         double tot = m + baseE;

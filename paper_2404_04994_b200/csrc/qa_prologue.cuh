@@ -4,7 +4,7 @@
 #include "qa_internal.cuh"
 
 struct QaPixelFlags {
-    bool neg, failed, widened;
+    bool neg, failed;
     int rounds, doublings;
 };
 
@@ -287,7 +287,6 @@ __device__ __forceinline__ void qa_prologue_pixel(const double *__restrict__ sCg
     if (neg) rounds = qa_qp_clamp<N>(sC, nc, closed, (double)args.N_hat, args.general_qp != 0, x, failed);
     // S4
     int doublings = 0;
-    bool widened = false;
     if (args.alg == QA_ALG_BRUTE_FORCE) {
 #pragma unroll
         for (int i = 0; i < N; ++i) {
@@ -313,20 +312,13 @@ __device__ __forceinline__ void qa_prologue_pixel(const double *__restrict__ sCg
                 ++doublings;
                 continue;
             }
-            widened = true;  // R5 fallback: {lo-1 .. lo+2} n [0, inf)
-#pragma unroll
-            for (int i = 0; i < N; ++i) {
-                const double fl = floor(x[i]);
-                const int32_t lo = fl > 0.0 ? (int32_t)fl : 0;
-                base[i] = lo > 0 ? lo - 1 : 0;
-                cnt[i] = lo + 2 - base[i] + 1;
-            }
+            // t = 1 is the closed default set, never empty for a feasible x (sum lo <= sum x = N_hat < sum lo + n up to
+            // rounding << 1; reading R5).  Were it empty, the search reports an empty set (N = -1, E = inf).
             break;
         }
     }
     fl.neg = neg;
     fl.failed = failed;
-    fl.widened = widened;
     fl.rounds = rounds;
     fl.doublings = doublings;
 }

@@ -14,8 +14,8 @@ import torch
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def header_functions():
-    src = open(os.path.join(ROOT, "include", "qarray_b200.h")).read()
+def header_functions(files=("qarray_b200.h", "qarray_b200_aids.h")):
+    src = "".join(open(os.path.join(ROOT, "include", f)).read() for f in files)
     return sorted(set(re.findall(r"QA_API[^;(]*?\b(qa_[a-z0-9_]+)\s*\(", src)))
 
 
@@ -31,6 +31,11 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     out = subprocess.run(["nm", "-D", "--defined-only", api.LIB_PATH], capture_output=True, text=True).stdout
     exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l)
     assert exported == names, "the library must export exactly the C ABI"
+    # the product header holds no measurement aid
+    prod = header_functions(("qarray_b200.h",))
+    for aid in ("qa_measure_fp64_rate", "qa_set_kernel_timing", "qa_get_kernel_timings", "qa_last_launch_plan",
+                "qa_last_launch_count", "qa_model_set_walk_variant"):
+        assert aid in names and aid not in prod
     assert b"sm_100a" in api.lib().qa_version()
 
 

@@ -180,8 +180,11 @@ def test_P4_energy_definition_offset_and_local_minimum():
         assert e >= 0
         assert np.isclose(e, 0.5 * d @ np.linalg.solve(w.C_dd, d), rtol=1e-12)
         assert np.isclose(m.free_energy_eq4(nc, N), e - 0.5 * nc @ Minv @ nc, rtol=1e-11, atol=1e-12)
-        # an asymmetric probe catches a transposed / half-summed M
-        assert np.isclose(m.energy(nc, N), m.energy(nc, N.copy()))
+        # an asymmetric probe catches a transposed / half-summed M: E(N + e_i) - E(N) = (M d)_i + 1/2 M_ii, one dot only
+        i = int(rng.integers(0, 6))
+        N2 = N.copy()
+        N2[i] += 1
+        assert np.isclose(m.energy(nc, N2) - e, (Minv @ d)[i] + 0.5 * Minv[i, i], rtol=1e-10, atol=1e-12)
     assert m.energy(np.array([1.0, 2, 0, 3, 1, 1]), np.array([1, 2, 0, 3, 1, 1], dtype=np.int32)) == 0.0
     rb = m.ground_state(w.Vg, algorithm="brute", n_max=4)
     for p in range(w.P):
@@ -433,6 +436,59 @@ def test_qp_used_only_when_needed_and_flagged():
     assert (r["x"][need].min(1) == 0.0).all()       # clamped components are exactly 0 (R3)
 
 
+def test_closed_qp_single_free_dot_is_bitwise_N_hat():
+    """Reading R3: when all dots but one clamp, 1^T x = N_hat fixes the free component: exactly N_hat, bitwise (n >= 2);
+    the clamped components are exactly 0, and the point is the KKT point of the exhaustive enumeration."""
+    rng = np.random.default_rng(41)
+    hits = 0
+    for trial in range(40):
+        n = int(rng.integers(2, 8))
+        w = wl.random_open(n, n, 1, seed=2000 + trial)
+        m = oracle.Model(w.C_dd, w.C_gd)
+        M = np.linalg.inv(w.C_dd)
+        f = int(rng.integers(0, n))
+        c = rng.uniform(-6.0, -3.0, size=n)          # everything strongly repelled ...
+        c[f] = rng.uniform(0.5, 3.0)                 # ... except one dot
+        N_hat = float(rng.integers(1, 5))
+        x, it, kkt = m.qp(c, closed=True, N_hat=N_hat)
+        want = _qp_by_active_set_enumeration(M, c, True, N_hat)
+        assert it > 0 and kkt < 1e-11 and np.allclose(x, want, atol=1e-10)
+        if (want > 1e-9).sum() == 1:
+            hits += 1
+            assert x[f] == N_hat                      # bitwise
+            assert (np.delete(x, f) == 0.0).all()
+    assert hits >= 30
+    # the same through the whole pixel pipeline: closed chain, one gate far positive, the others far negative
+    C_dd, C_gd = chain(4, 3)
+    m = oracle.Model(C_dd, C_gd)
+    target = np.array([[-5.0, 2.0, -5.0, -5.0], [-4.0, -4.0, -4.0, 1.5]])
+    r = m.ground_state(target @ np.linalg.inv(C_gd).T, regime="closed", N_hat=3)
+    assert r["x"].tolist() == [[0.0, 3.0, 0.0, 0.0], [0.0, 0.0, 0.0, 3.0]]
+    assert r["N"].tolist() == [[0, 3, 0, 0], [0, 0, 0, 3]]
+
+
+def test_R5_closed_default_set_is_never_empty():
+    """Reading R5: at t = 1 the kept set is the closed default set; for a feasible continuous minimum (x >= 0, sum x =
+    N_hat up to rounding) sum floor(x) <= N_hat <= sum floor(x) + n, so it is never empty and no wider set is needed.
+    Checked on the oracle's own x over analytic and QP pixels, Maxwell and general SPD c_dd, and through the flags."""
+    for seed, gen in ((1, wl.random_open), (2, wl.random_open), (3, wl.random_general)):
+        for n in (1, 2, 5, 8):
+            if n == 1 and gen is wl.random_general:
+                continue
+            w = gen(n, n, 800, seed=300 + 10 * seed + n, lo=-1.5, hi=3.0)
+            m = oracle.Model(w.C_dd, w.C_gd)
+            for N_hat in (0, 1, n, 2 * n + 1):
+                r = m.ground_state(w.Vg, regime="closed", N_hat=N_hat)
+                x = r["x"]
+                assert (x >= 0).all() and np.allclose(x.sum(1), N_hat, atol=1e-9)
+                lo = np.floor(x).sum(1)
+                assert ((lo <= N_hat) & (N_hat <= lo + n)).all()
+                assert (r["flags"] & (oracle.FLAG_EMPTY | oracle.FLAG_WIDENED | oracle.FLAG_QP_FAIL)).max() == 0
+                assert (r["N"].sum(1) == N_hat).all() and (r["n_scored"] >= 1).all()
+                rt = m.ground_state(w.Vg, regime="closed", N_hat=N_hat, algorithm="thresholded", t=0.0)
+                assert (rt["flags"] & oracle.FLAG_EMPTY).max() == 0 and (rt["N"].sum(1) == N_hat).all()
+
+
 # ---------------------------------------------------------------------------------------------------------- P12
 def test_P12_closed_two_dot_detuning_axis():
     """Closed double dot, N_hat = 1, M = [[a,c],[c,a']]: E(1,0) = E(0,1) <=> (a-c) u1 - (a'-c) u2 = (a-a')/2.  For
@@ -507,6 +563,9 @@ def test_R8_sensor_closed_forms():
     """L149 + Eq. (3): array dots solved on the sub-blocks; sensor carrier number = integer nearest to the 1-D
     parabola's vertex s* (Theorem E.1 in one dimension), clamped at 0; V_s = [M (N - N_c)]_s.  numpy route."""
     w = wl.config3(30, 30)
+    # config 3 keeps its sensor gate fixed (the sensor's carrier number is 1 on the whole sweep); ramp it here so that
+    # the two-way choice of the sensor step is exercised across several transitions
+    w.Vg[:, 4] = np.linspace(0.0, 3.0, w.P) / w.C_gd[4, 4]
     out = oracle.sensor_ground_state(w.C_dd, w.C_gd, w.sensor_dots, w.Vg)
     D = [0, 1, 2, 3]
     sub = oracle.Model(w.C_dd[np.ix_(D, D)], w.C_gd[D, :])
@@ -521,7 +580,35 @@ def test_R8_sensor_closed_forms():
     assert np.array_equal(out["N"][keep, 4], want[keep])
     d = out["N"] - nc
     assert np.allclose(out["Vs"][:, 0], d @ M[4, :], rtol=1e-11, atol=1e-13)
-    assert len(np.unique(out["N"][:, 4])) >= 1 and out["Vs"].std() > 0
+    assert len(np.unique(out["N"][:, 4])) >= 2 and out["Vs"].std() > 0
+    # margin of the two-way choice: |e(c0+1) - e(c0)| with e(c) = (c - u) y + 1/2 M_ss (c - u)^2, i.e. M_ss |c0 + 1/2 - s*|
+    c0 = np.floor(np.maximum(sstar, 0.0))
+    assert np.allclose(out["sgap"][:, 0], M[4, 4] * np.abs(c0 + 0.5 - sstar), rtol=1e-9, atol=1e-12)
+
+
+def test_R8_two_sensors_at_non_trailing_indices():
+    """Reading R8 with several sensors: 6 dots, sensors {2, 5} (ns > 1, sensor indices between array dots).  Each sensor is
+    rounded independently with the OTHER sensor at its continuous value (d = 0); V_s uses every final N.  numpy route."""
+    w = wl.random_open(6, 7, 400, seed=77, lo=-0.3, hi=2.6)
+    sens = (2, 5)
+    D = [0, 1, 3, 4]
+    out = oracle.sensor_ground_state(w.C_dd, w.C_gd, sens, w.Vg)
+    sub = oracle.Model(w.C_dd[np.ix_(D, D)], w.C_gd[D, :])
+    rs = sub.ground_state(w.Vg)
+    assert np.array_equal(out["N"][:, D], rs["N"]) and np.array_equal(out["E"], rs["E"])
+    M = np.linalg.inv(w.C_dd)
+    nc = w.Vg @ w.C_gd.T
+    dD = out["N"][:, D] - nc[:, D]
+    for a, s_ in enumerate(sens):
+        sstar = nc[:, s_] - (dD @ M[s_, D]) / M[s_, s_]
+        keep = np.abs(sstar - np.floor(sstar) - 0.5) > 1e-9
+        want = np.floor(np.maximum(sstar, 0.0) + 0.5).astype(np.int32)
+        assert np.array_equal(out["N"][keep, s_], want[keep])
+        assert len(np.unique(out["N"][:, s_])) >= 2
+        c0 = np.floor(np.maximum(sstar, 0.0))
+        assert np.allclose(out["sgap"][:, a], M[s_, s_] * np.abs(c0 + 0.5 - sstar), rtol=1e-9, atol=1e-12)
+    d = out["N"] - nc
+    assert np.allclose(out["Vs"], d @ M[list(sens), :].T, rtol=1e-11, atol=1e-13)
 
 
 def test_brute_force_is_the_definition_on_the_box():
