@@ -1,0 +1,588 @@
+// qa_kernels_fused_open.cu -- the whole path S1-S7 (S8 for a model with sensor dots) of SURVEY.md section 8(a) in ONE kernel
+// for OPEN arrays with n <= 8 dots and a BINARY candidate set: the default algorithm (lo + {0,1}^n, L123-L127) and the
+// thresholded one (lo/round + a subset of the free dots, Eq. (9)).  This is the kernel of the dataset batch
+// (BASELINE.json configs[4]: 256 arrays x 128x128 pixels x {default, t = 0.2, t = 0.5}); blockIdx.y selects the model.
+//
+// What bounds it: V_g is the only HBM read (8 g bytes per pixel), N*, E(N*) the only writes, so the
+// floor is HBM (104 B per pixel at n = g = 8); the arithmetic next to it is ~200 FP64 instructions of per-pixel prologue
+// and epilogue (N_c: n g FMA, M d0: n^2 FMA, E(N*) from the definition: n^2 + n FMA) plus the candidate walk.  Every FMA
+// of the prologue takes one operand from a per-MODEL matrix, i.e. a warp-uniform value that has to come out of shared
+// memory (the model differs per CTA, so the constant bank is not available): a broadcast LDS.128 returns 512 B for two
+// operands, four SM cycles of the shared-memory pipe, while the FP64 pipe needs 2 cycles per scheduler for the two FMAs
+// -- with one pixel per thread the kernel would be bound by shared-memory return bandwidth at 1/4 of the FP64 rate.  Hence
+// TWO pixels per thread everywhere (prologue, walk, epilogue): every uniform operand fetched serves two FMAs / DADDs.
+//
+// Register discipline: nothing in the common path is dynamically indexed, so nothing lives in local memory.  The QP
+// (L106, reading R3) is solved in closed form in registers for one to three clamped dots (all but 3 in 10^5 pixels of the
+// batch); larger active sets and non-Maxwell models are redone after the kernel's own stores by a __noinline__ function
+// with the general solver (fo_slow_pixel), whose work arrays never touch the frame of the common path.
+//
+// Candidate walk.
+//   default:      the static counting-order walk of qa_kernels_walk.cu over all 2^n patterns, two pixels at once (3 FP64
+//                 instructions per candidate and pixel, one table entry per candidate for both pixels).
+//   thresholded:  the number of free dots k differs from pixel to pixel (2^k candidates: 4.3 on average at t = 0.2, 25.6
+//                 at t = 0.5, but up to 256), so a warp of neighbouring pixels would run at the pace of its largest set.  The
+//                 256 pixels of a CTA are therefore bucket-sorted by k in shared memory and every thread walks two
+//                 pixels of (nearly) equal k.  The walk is the counting-order walk restricted to the free dots: with the
+//                 free dots f_0 < f_1 < .. (bit positions) the step st-1 -> st sets free bit j = ctz(st) and clears the
+//                 free bits below it, so the linear part moves by c_j = h_{f_j} - sum_{i<j} h_{f_i} (stored per pixel in
+//                 shared memory, read with a warp-uniform j) and the bit pattern by an XOR mask; ascending st is ascending
+//                 pattern, so the strict '<' keeps the lexicographically smallest N among equal energies (reading R6).
+//   The winner's energy E(N*) is recomputed from the definition (Eq. (C1)) by the thread that owns the pixel.
+#include "qa_internal.cuh"
+#include "qa_prologue.cuh"
+
+namespace {
+
+constexpr int FO_THREADS = 128;
+constexpr int FO_PX = 2;                        // pixels per thread
+constexpr int FO_PIX = FO_THREADS * FO_PX;      // pixels per CTA
+
+__host__ __device__ constexpr int fo_ctz(int k)
+{
+    int j = 0;
+    while (((k >> j) & 1) == 0) ++j;
+    return j;
+}
+
+// Sensor step S8 on its own frame (single-model calls with sensor dots only).
+__device__ __noinline__ void fo_sensor(const QaDevModel *__restrict__ mdl, const double *__restrict__ Vg, int64_t p,
+                                       const int32_t *Ns, int32_t *__restrict__ outN, double *__restrict__ outVs)
+{
+    qa_sensor_pixel(mdl, Vg, p, Ns, outN, outVs);
+}
+
+// Open-array QP of one pixel in registers: clamp-only monotone active set (reading R3), closed form for |A| <= 3.
+// x holds the analytic minimum (= c) on entry.  Returns the number of rounds.  slow = true: more than three clamped dots or a
+// c_dd with a positive off-diagonal -- the pixel is redone by fo_slow_pixel at the end of the kernel (x is then unusable).
+template <int N>
+__device__ __forceinline__ int fo_qp_open(const double *__restrict__ sC, const double (&c)[N], int general, double (&x)[N],
+                                          bool &failed, bool &slow)
+{
+    unsigned A = 0;
+    int rounds = 0;
+    slow = general != 0;
+    double scale = 1.0;
+#pragma unroll
+    for (int i = 0; i < N; ++i) scale = fmax(scale, fabs(c[i]));
+    while (!slow) {
+        unsigned neg = 0;
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+            if (x[i] < 0.0) neg |= 1u << i;
+        neg &= ~A;
+        if (!neg) break;
+        A |= neg;
+        ++rounds;
+        const int na = __popc(A);
+        if (na == N) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) x[i] = 0.0;
+            break;
+        }
+        if (na > 3) {
+            slow = true;
+            break;
+        }
+        if (!qa_qp_small_open<N>(sC, c, A, scale, x)) failed = true;
+    }
+    return rounds;
+}
+
+template <int N, bool THR>
+struct FoSort {  // thresholded: bookkeeping of the bucket sort and the walk
+    unsigned long long xm[THR ? FO_PIX : 1];  // XOR masks of the steps, 8 bits per free dot
+    unsigned short order[THR ? FO_PIX : 1];   // pixel slots sorted by the number of free dots, descending
+    unsigned char kfree[THR ? FO_PIX : 1];    // number of free dots
+    unsigned char wkey[THR ? FO_PIX : 1];     // winning pattern
+    int bucket[16];
+};
+
+template <int N, bool THR>
+struct FoSmem {
+    double MT[N * N];          // MT[j*N + i] = M[i][j]: the N values a column step needs are contiguous
+    double C[N * N];           // c_dd, row-major (QP)
+    double T[1 << N];          // pair table of the bit patterns: T[b] = QL[b] (bit j <-> dot N-1-j)
+    double nc[N][FO_PIX];      // N_c of every pixel slot, parked during the walk (registers: 4 CTAs per SM)
+    int32_t base[N][FO_PIX];   // ... and the base point
+    double cs[THR ? N : 1][FO_PIX];     // thresholded: c_j of the compacted free dots, per pixel slot
+    union {                    // C_gd is dead after S1 (a barrier separates it from the sort's first write)
+        double CgT[QA_MAXG * N];   // CgT[k*N + i] = C_gd[i][k]
+        FoSort<N, THR> sort;
+    };
+};
+
+// A pixel the register path defers (more than three clamped dots, or a c_dd with a positive off-diagonal: 3 in 10^5
+// pixels of the dataset batch): the whole path S1-S7 once more, by one thread, with the general QP solver of
+// qa_prologue.cuh, the same h / c_j / pair-table walk in ascending pattern order, and E(N*) from the definition.
+// __noinline__, called after the kernel's own stores: its work arrays never touch the frame of the common path.
+template <int N, bool THR>
+__device__ __noinline__ void fo_slow_pixel(const double *__restrict__ MT, const double *__restrict__ C,
+                                           const double *__restrict__ T,
+                                           const QaDevModel *__restrict__ mdl, const double *__restrict__ Vg, int64_t gp,
+                                           QaCallArgs args, int32_t *__restrict__ outN, double *__restrict__ outE,
+                                           double *__restrict__ xcont, double *__restrict__ outVs, int *stat)
+{
+    const int g = mdl->g;
+    double nc[N], x[N], d0[N], hp[N], cs[N];
+    int32_t base[N];
+    for (int i = 0; i < N; ++i) {
+        double acc = 0.0;
+        for (int k = 0; k < g; ++k) acc = fma(mdl->Cgd[i * QA_MAXG + k], __ldg(Vg + gp * g + k), acc);
+        nc[i] = acc;
+        x[i] = acc;
+    }
+    bool failed = false;
+    const int rounds = qa_qp_clamp<N>(C, nc, false, 0.0, args.general_qp != 0, x, failed);
+    unsigned fm = 0;
+    for (int i = 0; i < N; ++i) {
+        int32_t cn;
+        qa_floor_ceil(x[i], args.t, THR, base[i], cn);
+        if (cn == 2) fm |= 1u << (N - 1 - i);
+        d0[i] = (double)base[i] - nc[i];
+    }
+    for (int i = 0; i < N; ++i) {
+        double gi = 0.0;
+        for (int j = 0; j < N; ++j) gi = fma(MT[j * N + i], d0[j], gi);
+        hp[N - 1 - i] = gi + 0.5 * MT[i * N + i];
+    }
+    unsigned long long xm = 0;
+    int kf = 0;
+    {
+        double pre = 0.0;
+        unsigned low = 0;
+        for (int b = 0; b < N; ++b)
+            if ((fm >> b) & 1u) {
+                cs[kf] = hp[b] - pre;
+                pre += hp[b];
+                xm |= (unsigned long long)((1u << b) | low) << (8 * kf);
+                low |= 1u << b;
+                ++kf;
+            }
+    }
+    double s = 0.0, best = 0.0;
+    unsigned key = 0, bkey = 0;
+    for (unsigned st = 1; st < (1u << kf); ++st) {
+        const int j = __ffs(st) - 1;
+        s += cs[j];
+        key ^= (unsigned)(xm >> (8 * j)) & 0xffu;
+        const double e = s + T[key];
+        if (e < best) {
+            best = e;
+            bkey = key;
+        }
+    }
+    int32_t Ns[N];
+    double d[N];
+    for (int i = 0; i < N; ++i) {
+        Ns[i] = base[i] + (int32_t)((bkey >> (N - 1 - i)) & 1u);
+        d[i] = (double)Ns[i] - nc[i];
+    }
+    double Ed = 0.0;
+    for (int i = 0; i < N; ++i) {
+        double row = 0.0;
+        for (int j = 0; j < N; ++j) row = fma(MT[j * N + i], d[j], row);
+        Ed = fma(d[i], row, Ed);
+    }
+    outE[gp] = 0.5 * Ed;
+    if (mdl->ns == 0) {
+        for (int i = 0; i < N; ++i) outN[gp * N + i] = Ns[i];
+    } else {
+        qa_sensor_pixel(mdl, Vg, gp, Ns, outN, outVs);
+    }
+    if (xcont)
+        for (int i = 0; i < N; ++i) xcont[gp * N + i] = x[i];
+    stat[0] = rounds;
+    stat[1] = failed ? 1 : 0;
+    stat[2] = kf;
+}
+
+// Rank of the calling thread among the threads of the CTA that pass the same `key` (0..15), any order: one shared-memory
+// atomic per distinct key and warp instead of one per thread (all pixels of a CTA often share a key).
+__device__ __forceinline__ int fo_bucket_rank(int *bucket, int key)
+{
+    const unsigned peers = __match_any_sync(0xffffffffu, key);
+    const unsigned lane = threadIdx.x & 31u;
+    const int leader = __ffs(peers) - 1;
+    int start = 0;
+    if ((int)lane == leader) start = atomicAdd(&bucket[key], __popc(peers));
+    start = __shfl_sync(0xffffffffu, start, leader);
+    return start + __popc(peers & ((1u << lane) - 1u));
+}
+
+template <int N, bool THR>
+__global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDevModel *const *__restrict__ models,
+                                                                   const double *__restrict__ Vg, int64_t P,
+                                                                   QaCallArgs args, int32_t *__restrict__ outN,
+                                                                   double *__restrict__ outE, double *__restrict__ xcont,
+                                                                   double *__restrict__ outVs, qa_stats *stats)
+{
+    __shared__ __align__(16) FoSmem<N, THR> sm;
+    const QaDevModel *__restrict__ mdl = models[blockIdx.y];
+    const int g = mdl->g;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < N * N; e += FO_THREADS) {
+        sm.MT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
+        sm.C[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
+    }
+    for (int e = tid; e < N * g; e += FO_THREADS) sm.CgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
+    for (int k = tid; k < (1 << N); k += FO_THREADS) sm.T[k] = mdl->QL[k];
+    const int ns = mdl->ns;
+    __syncthreads();
+
+    // ---- S1-S4 for the thread's two pixels: slot = tid + px * FO_THREADS (coalescing: consecutive threads, consecutive rows)
+    int64_t gp[FO_PX];
+    bool live[FO_PX];
+    double nc[FO_PX][N], hp[FO_PX][N];   // hp[b]: energy increment of raising dot N-1-b at the base point
+    unsigned freem[FO_PX];               // bit b set: dot N-1-b has two candidate values
+    int rounds[FO_PX], rk[FO_PX];
+    bool negf[FO_PX], failed[FO_PX], slowf[FO_PX];
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px) {
+        const int64_t p = (int64_t)blockIdx.x * FO_PIX + px * FO_THREADS + tid;
+        live[px] = p < P;
+        gp[px] = (int64_t)blockIdx.y * P + (live[px] ? p : P - 1);
+#pragma unroll
+        for (int i = 0; i < N; ++i) nc[px][i] = 0.0;
+    }
+    {   // S1: N_c,i = fma(C_gd[i,k], V[k], acc), k ascending (R1).  Chunks of 8 gates: the 16 loads of a chunk are issued
+        // before its FMAs (the rows come from HBM: one round trip per chunk, not per gate).
+        const double *v0 = Vg + gp[0] * g, *v1 = Vg + gp[1] * g;
+        const bool vec = (g & 1) == 0 && (reinterpret_cast<uintptr_t>(Vg) & 15u) == 0;
+        for (int k0 = 0; k0 < g; k0 += 8) {
+            double a[8], b[8];
+            if (vec) {
+#pragma unroll
+                for (int k = 0; k < 8; k += 2) {
+                    double2 ta = make_double2(0.0, 0.0), tb = ta;
+                    if (k0 + k < g) {
+                        ta = __ldg(reinterpret_cast<const double2 *>(v0 + k0 + k));
+                        tb = __ldg(reinterpret_cast<const double2 *>(v1 + k0 + k));
+                    }
+                    a[k] = ta.x, a[k + 1] = ta.y, b[k] = tb.x, b[k + 1] = tb.y;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    a[k] = k0 + k < g ? __ldg(v0 + k0 + k) : 0.0;
+                    b[k] = k0 + k < g ? __ldg(v1 + k0 + k) : 0.0;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (k0 + k < g) {
+#pragma unroll
+                    for (int i = 0; i < N; ++i) {
+                        const double cg = sm.CgT[(k0 + k) * N + i];
+                        nc[0][i] = fma(cg, a[k], nc[0][i]);
+                        nc[1][i] = fma(cg, b[k], nc[1][i]);
+                    }
+                }
+            }
+        }
+    }
+    double d0[FO_PX][N];
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px) {
+        // S2 + S3
+        double x[N];
+        bool neg = false;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            x[i] = nc[px][i];
+            neg |= x[i] < 0.0;
+        }
+        rounds[px] = 0;
+        rk[px] = 0;
+        failed[px] = false;
+        slowf[px] = false;
+        if (neg) rounds[px] = fo_qp_open<N>(sm.C, nc[px], args.general_qp, x, failed[px], slowf[px]);
+        negf[px] = neg;
+        // S4 (Eq. (9), readings R4 / R10)
+        unsigned fm = 0;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            int32_t cn, bs;
+            qa_floor_ceil(x[i], args.t, THR, bs, cn);
+            if (cn == 2) fm |= 1u << (N - 1 - i);
+            d0[px][i] = (double)bs - nc[px][i];
+            // N_c and the base point wait in shared memory while the gradient and the walk have the registers
+            sm.nc[i][px * FO_THREADS + tid] = nc[px][i];
+            sm.base[i][px * FO_THREADS + tid] = bs;
+        }
+        freem[px] = fm;
+        if (xcont && live[px] && !slowf[px]) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) xcont[gp[px] * N + i] = x[i];
+        }
+    }
+    {   // base-point gradient grad = M d0 (row i: j ascending), h_i = grad_i + 1/2 M_ii
+        double grad[FO_PX][N];
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px)
+#pragma unroll
+            for (int i = 0; i < N; ++i) grad[px][i] = 0.0;
+#pragma unroll
+        for (int j = 0; j < N; ++j) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                const double mij = sm.MT[j * N + i];
+                grad[0][i] = fma(mij, d0[0][j], grad[0][i]);
+                grad[1][i] = fma(mij, d0[1][j], grad[1][i]);
+            }
+        }
+#pragma unroll
+        for (int b = 0; b < N; ++b) {
+            const double hm = 0.5 * sm.MT[(N - 1 - b) * N + (N - 1 - b)];
+            hp[0][b] = grad[0][N - 1 - b] + hm;
+            hp[1][b] = grad[1][N - 1 - b] + hm;
+        }
+    }
+
+    asm volatile("" ::: "memory");
+    // ---- S5-S6
+    unsigned win[FO_PX];
+    if constexpr (!THR) {
+        // counting-order walk over all 2^N patterns, both pixels at once (qa_kernels_walk.cu).  A real loop over chunks of
+        // 2^LB patterns (the fully unrolled walk is 60 KB of code and stalls on instruction fetch): inside a chunk every
+        // index is static; the step into chunk i sets bit LB + ctz(i), picked from registers by a short select chain.
+        constexpr int LB = N < 4 ? N : 4;
+        constexpr int NHI = N - LB;
+        double cl[FO_PX][LB], ch[FO_PX][NHI > 0 ? NHI : 1], s[FO_PX], m[FO_PX];
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            double pre = 0.0;
+#pragma unroll
+            for (int j = 0; j < N; ++j) {
+                if (j < LB)
+                    cl[px][j] = hp[px][j] - pre;
+                else
+                    ch[px][j - LB] = hp[px][j] - pre;
+                pre += hp[px][j];
+            }
+            s[px] = 0.0;
+            m[px] = 0.0;
+            win[px] = 0;
+        }
+#pragma unroll 1
+        for (int i = 0; i < (1 << NHI); ++i) {
+            const double *__restrict__ T = sm.T + (i << LB);
+            const unsigned kb = (unsigned)i << LB;
+            if (i > 0) {
+                const double q = T[0];
+#pragma unroll
+                for (int px = 0; px < FO_PX; ++px) {
+                    double c = ch[px][NHI > 0 ? NHI - 1 : 0];
+#pragma unroll
+                    for (int j = NHI - 2; j >= 0; --j)
+                        if ((i >> j) & 1) c = ch[px][j];
+                    s[px] += c;
+                    const double e = s[px] + q;
+                    if (e < m[px]) {
+                        m[px] = e;
+                        win[px] = kb;
+                    }
+                }
+            }
+#pragma unroll
+            for (int w = 1; w < (1 << LB); ++w) {
+                const double q = T[w];
+#pragma unroll
+                for (int px = 0; px < FO_PX; ++px) {
+                    s[px] += cl[px][fo_ctz(w)];
+                    const double e = s[px] + q;
+                    if (e < m[px]) {
+                        m[px] = e;
+                        win[px] = kb + w;
+                    }
+                }
+            }
+        }
+    } else {
+        // compaction of the free dots (ascending bit position), bucket sort of the CTA's pixels by k, walk, hand back
+        __syncthreads();  // every warp is done with C_gd: its storage becomes the sort's
+        if (tid < 16) sm.sort.bucket[tid] = 0;
+        __syncthreads();
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            const int slot = px * FO_THREADS + tid;
+            double pre = 0.0;
+            int jj = 0;
+            unsigned low = 0;
+            unsigned long long xm = 0;
+#pragma unroll
+            for (int b = 0; b < N; ++b) {
+                if ((freem[px] >> b) & 1u) {
+                    sm.cs[jj][slot] = hp[px][b] - pre;
+                    pre += hp[px][b];
+                    xm |= (unsigned long long)((1u << b) | low) << (8 * jj);
+                    low |= 1u << b;
+                    ++jj;
+                }
+            }
+            const int kf = live[px] ? jj : 0;
+            sm.sort.xm[slot] = xm;
+            sm.sort.kfree[slot] = (unsigned char)kf;
+            sm.sort.wkey[slot] = 0;
+            rk[px] = fo_bucket_rank(sm.sort.bucket, N - kf);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            const int slot = px * FO_THREADS + tid;
+            const int kf = sm.sort.kfree[slot];
+            int start = 0;
+#pragma unroll
+            for (int bkt = 0; bkt <= N; ++bkt)
+                if (bkt < N - kf) start += sm.sort.bucket[bkt];
+            sm.sort.order[start + rk[px]] = (unsigned short)slot;
+        }
+        __syncthreads();
+        // thread tid walks the pixels of rank tid (large sets first) and FO_PIX-1-tid (small sets): balanced pairs
+#pragma unroll 1
+        for (int half = 0; half < 2; ++half) {
+            const int slot = sm.sort.order[half == 0 ? tid : FO_PIX - 1 - tid];
+            const unsigned nst = 1u << sm.sort.kfree[slot];
+            const unsigned long long xm = sm.sort.xm[slot];
+            double s = 0.0, best = 0.0;
+            unsigned key = 0, bkey = 0;
+            for (unsigned st = 1; st < nst; ++st) {
+                const int j = __ffs(st) - 1;
+                s += sm.cs[j][slot];
+                key ^= (unsigned)(xm >> (8 * j)) & 0xffu;
+                const double e = s + sm.T[key];
+                if (e < best) {
+                    best = e;
+                    bkey = key;
+                }
+            }
+            sm.sort.wkey[slot] = (unsigned char)bkey;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) win[px] = sm.sort.wkey[px * FO_THREADS + tid];
+    }
+
+    // (compiler barrier: without it the M values the gradient phase loaded are kept for the epilogue -- in local memory)
+    asm volatile("" ::: "memory");
+    // ---- S7 (+ S8): N* = base + bits of the winner; E(N*) = 1/2 d^T M d from the definition (Eq. (C1))
+    int32_t Ns[FO_PX][N];
+    double d[FO_PX][N];
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px)
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            Ns[px][i] = sm.base[i][px * FO_THREADS + tid] + (int32_t)((win[px] >> (N - 1 - i)) & 1u);
+            d[px][i] = (double)Ns[px][i] - sm.nc[i][px * FO_THREADS + tid];
+        }
+    double row[FO_PX][N];
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px)
+#pragma unroll
+        for (int i = 0; i < N; ++i) row[px][i] = 0.0;
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double mij = sm.MT[j * N + i];
+            row[0][i] = fma(mij, d[0][j], row[0][i]);
+            row[1][i] = fma(mij, d[1][j], row[1][i]);
+        }
+    }
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px) {
+        double Ed = 0.0;
+#pragma unroll
+        for (int i = 0; i < N; ++i) Ed = fma(d[px][i], row[px][i], Ed);
+        if (live[px]) {
+            outE[gp[px]] = 0.5 * Ed;
+            if (ns == 0) {
+                if constexpr (N % 4 == 0) {
+                    if ((reinterpret_cast<uintptr_t>(outN) & 15u) == 0) {
+#pragma unroll
+                        for (int i = 0; i < N; i += 4)
+                            *reinterpret_cast<int4 *>(outN + gp[px] * N + i) =
+                                make_int4(Ns[px][i], Ns[px][i + 1], Ns[px][i + 2], Ns[px][i + 3]);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < N; ++i) outN[gp[px] * N + i] = Ns[px][i];
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < N; ++i) outN[gp[px] * N + i] = Ns[px][i];
+                }
+            } else {  // S8: sensor dots in the full model (single-model calls only: gp = p)
+                int32_t Nl[N];
+#pragma unroll
+                for (int i = 0; i < N; ++i) Nl[i] = Ns[px][i];
+                fo_sensor(mdl, Vg, gp[px], Nl, outN, outVs);
+            }
+        }
+    }
+    // deferred pixels (see fo_slow_pixel): redone from scratch, overwriting what the register path stored
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px) {  // (unrolled: a dynamic px would put every per-pixel array in local memory)
+        if (live[px] && slowf[px]) {
+            int st3[3];
+            fo_slow_pixel<N, THR>(sm.MT, sm.C, sm.T, mdl, Vg, gp[px], args, outN, outE, xcont, outVs, st3);
+            rounds[px] = st3[0];
+            failed[px] = st3[1] != 0;
+            freem[px] = (1u << st3[2]) - 1u;  // only its population count is used below
+        }
+    }
+    if (stats) {
+        int64_t np = 0, nq = 0, nr = 0, nf = 0, ne = 0;
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            if (!live[px]) continue;
+            ++np;
+            nq += negf[px] ? 1 : 0;
+            nr += rounds[px];
+            nf += failed[px] ? 1 : 0;
+            ne += (int64_t)1 << __popc(freem[px]);
+        }
+        qa_warp_count(&stats->n_pixels, np);
+        qa_warp_count(&stats->n_qp_pixels, nq);
+        qa_warp_count(&stats->n_qp_rounds, nr);
+        qa_warp_count(&stats->n_qp_failed, nf);
+        qa_warp_count(&stats->n_candidates_enumerated, ne);
+        qa_warp_count(&stats->n_candidates_scored, ne);
+    }
+}
+
+template <int N>
+cudaError_t launch_fused_open_n(const QaDevModel *const *d_models, int n_models, const double *d_Vg, int64_t P,
+                                QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
+                                qa_stats *d_stats, cudaStream_t stream)
+{
+    const dim3 grid((unsigned)((P + FO_PIX - 1) / FO_PIX), (unsigned)n_models);
+    if (args.alg == QA_ALG_DEFAULT)
+        qa_fused_open_kernel<N, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats);
+    else
+        qa_fused_open_kernel<N, true><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// Open arrays, default or thresholded algorithm, n <= QA_FUSED_MAXN.  Arguments as qa_launch_fused_small.
+cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
+                                 QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
+                                 qa_stats *d_stats, cudaStream_t stream)
+{
+    qa_plan_add("qa_fused_open_kernel");
+    if (n_models > 65535 || args.closed || args.alg == QA_ALG_BRUTE_FORCE) return cudaErrorInvalidValue;
+#define CALL(NN) launch_fused_open_n<NN>(d_models, n_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats, stream)
+    switch (n) {
+        case 1: return CALL(1);
+        case 2: return CALL(2);
+        case 3: return CALL(3);
+        case 4: return CALL(4);
+        case 5: return CALL(5);
+        case 6: return CALL(6);
+        case 7: return CALL(7);
+        case 8: return CALL(8);
+        default: return cudaErrorInvalidValue;
+    }
+#undef CALL
+}

@@ -97,6 +97,53 @@ __device__ void qa_qp_eqp(const double *__restrict__ sC, const double *c, bool c
     }
 }
 
+// Open array, one to three clamped dots A (nearly every QP pixel of a sweep): y_A = -C_AA^-1 c_A from the explicit inverse of
+// the 1x1 / 2x2 / 3x3 block (registers only), x_F = c_F + C_FA y_A, x_A = 0 exactly (R3).  Returns false if a bound
+// multiplier y_A is negative beyond rounding (KKT violated).  c and x are fully unrolled: static register indices.
+template <int N>
+__device__ __forceinline__ bool qa_qp_small_open(const double *__restrict__ sC, const double *c, unsigned A, double scale,
+                                                 double *x)
+{
+    const int ia = __ffs(A) - 1;
+    const unsigned A2 = A & (A - 1);
+    const int ib = A2 ? __ffs(A2) - 1 : ia;
+    const unsigned A3 = A2 & (A2 - 1);
+    const int ic = A3 ? __ffs(A3) - 1 : ib;
+    double ca = 0.0, cb = 0.0, cc = 0.0;
+#pragma unroll
+    for (int f = 0; f < N; ++f) {
+        if (f == ia) ca = c[f];
+        if (f == ib) cb = c[f];
+        if (f == ic) cc = c[f];
+    }
+    double ya, yb = 0.0, yc = 0.0;
+    if (A3) {
+        const double a = sC[ia * N + ia], b = sC[ia * N + ib], cq = sC[ia * N + ic];
+        const double d = sC[ib * N + ib], e = sC[ib * N + ic], f = sC[ic * N + ic];
+        const double k00 = d * f - e * e, k01 = cq * e - b * f, k02 = b * e - cq * d;
+        const double k11 = a * f - cq * cq, k12 = b * cq - a * e, k22 = a * d - b * b;
+        const double det = a * k00 + b * k01 + cq * k02;
+        ya = -(k00 * ca + k01 * cb + k02 * cc) / det;
+        yb = -(k01 * ca + k11 * cb + k12 * cc) / det;
+        yc = -(k02 * ca + k12 * cb + k22 * cc) / det;
+    } else if (A2) {
+        const double Caa = sC[ia * N + ia], Cab = sC[ia * N + ib], Cbb = sC[ib * N + ib];
+        const double det = Caa * Cbb - Cab * Cab;
+        ya = (cb * Cab - ca * Cbb) / det;
+        yb = (ca * Cab - cb * Caa) / det;
+    } else {
+        ya = -ca / sC[ia * N + ia];
+    }
+#pragma unroll
+    for (int f = 0; f < N; ++f) {
+        double s = c[f] + sC[f * N + ia] * ya;
+        if (A2) s += sC[f * N + ib] * yb;
+        if (A3) s += sC[f * N + ic] * yc;
+        x[f] = ((A >> f) & 1u) ? 0.0 : s;  // clamped components are exactly 0 (R3)
+    }
+    return !(ya < -1e-9 * scale || yb < -1e-9 * scale || yc < -1e-9 * scale);  // KKT: bound multipliers must be >= 0
+}
+
 // Phase 1 (every c_dd): the monotone clamp-only active set described above.  For a Maxwell c_dd it ends at the KKT point.
 // Phase 2 (only when c_dd has a positive off-diagonal, `general`): phase 1 still ends at a feasible x that minimises the
 // objective on its face x_A = 0, but a bound multiplier may be negative; from there the textbook primal active-set method
@@ -132,34 +179,8 @@ __device__ int qa_qp_clamp(const double *__restrict__ sC, const double *c, bool 
             if (closed) failed = true;
             break;
         }
-        if (!general && !closed && __popc(A) <= 2) {
-            // one or two clamped dots of an open array (nearly every QP pixel of a sweep): the 1x1 / 2x2 system in closed
-            // form, registers only -- y_A = -C_AA^-1 c_A, x_F = c_F + C_FA y_A
-            const int ia = __ffs(A) - 1;
-            const unsigned A2 = A & (A - 1);
-            const int ib = A2 ? __ffs(A2) - 1 : ia;
-            double ca = 0.0, cb = 0.0;
-#pragma unroll
-            for (int f = 0; f < N; ++f) {
-                if (f == ia) ca = c[f];
-                if (f == ib) cb = c[f];
-            }
-            double ya, yb = 0.0;
-            if (A2) {
-                const double Caa = sC[ia * N + ia], Cab = sC[ia * N + ib], Cbb = sC[ib * N + ib];
-                const double det = Caa * Cbb - Cab * Cab;
-                ya = (cb * Cab - ca * Cbb) / det;
-                yb = (ca * Cab - cb * Caa) / det;
-            } else {
-                ya = -ca / sC[ia * N + ia];
-            }
-            if (ya < -1e-9 * scale || yb < -1e-9 * scale) failed = true;  // KKT: bound multipliers must be >= 0
-#pragma unroll
-            for (int f = 0; f < N; ++f) {
-                double s = c[f] + sC[f * N + ia] * ya;
-                if (A2) s += sC[f * N + ib] * yb;
-                x[f] = ((A >> f) & 1u) ? 0.0 : s;  // clamped components are exactly 0 (R3)
-            }
+        if (!general && !closed && __popc(A) <= 3) {
+            if (!qa_qp_small_open<N>(sC, c, A, scale, x)) failed = true;
             continue;
         }
         qa_qp_eqp<N>(sC, c, closed, Nhat, A, x, r);

@@ -60,9 +60,10 @@ def check(api, w, variant=None, **kw):
 def test_config1_open_double_dot_default_and_brute(api):
     w = wl.config1(100, 100)
     rep, g, o = check(api, w, algorithm="default")
-    assert g["plan"][0] == ["qa_fused_small_kernel"]
+    assert g["plan"][0] == ["qa_fused_open_kernel"]
     assert st_zero_qp(g)
-    check(api, w, algorithm="brute", n_max=5)
+    rep, g, o = check(api, w, algorithm="brute", n_max=5)
+    assert g["plan"][0] == ["qa_fused_small_kernel"]
 
 
 def st_zero_qp(g):
@@ -220,7 +221,7 @@ def test_all_sizes_default_open(api, n):
     w = wl.random_open(n, n + (n % 3), 301 if n <= 10 else (67 if n <= 13 else 37), seed=50 + n)
     rep, g, o = check(api, w, algorithm="default")
     if n <= 8:   # the one-kernel path above; the three-kernel path (static walk) below
-        assert g["plan"][0] == ["qa_fused_small_kernel"]
+        assert g["plan"][0] == ["qa_fused_open_kernel"]
         rep, g0, o = check(api, w, variant=0, algorithm="default")
         assert g0["plan"][0] == ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"]
         assert np.array_equal(g["N"], g0["N"])
@@ -333,7 +334,7 @@ def test_batch_equals_loop_and_oracle(api):
                dict(algorithm="default", regime="closed", N_hat=8)):
         rb = batch.ground_state(Vg, want_xcont=True, want_stats=True, **kw)
         torch.cuda.synchronize()
-        assert api.last_launch_plan()[0] == ["qa_fused_small_kernel"]
+        assert api.last_launch_plan()[0] == ["qa_fused_small_kernel" if kw.get("regime") == "closed" else "qa_fused_open_kernel"]
         tot = 0
         for j, (w, m) in enumerate(zip(wls, models)):
             r1 = m.ground_state(Vg[j], **kw)
