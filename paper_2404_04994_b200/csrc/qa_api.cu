@@ -263,7 +263,7 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     {
         const double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n) : std::pow(2.0, (double)n);
         if (n <= QA_FUSED_MAXN && !closed && alg != QA_ALG_BRUTE_FORCE && variant != 0) {  // binary set of an open array
-            QA_CUDA(qa_launch_fused_open(m->dev_self, 1, n, d_Vg, P, a, d_N, d_E, d_xcont, m->ns > 0 ? d_Vsensor : nullptr,
+            QA_CUDA(qa_launch_fused_open(m->dev_self, 1, n, m->g, d_Vg, P, a, d_N, d_E, d_xcont, m->ns > 0 ? d_Vsensor : nullptr,
                                          d_stats, stream));
             timing_mark(stream);
             return QA_OK;
@@ -624,7 +624,7 @@ qa_status qa_ground_state_batch(const qa_batch *bt, const double *d_Vg, int64_t 
     if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
     QaCallArgs a{closed, N_hat, (int)alg, t, n_max, bt->general};
     if (!closed && alg != QA_ALG_BRUTE_FORCE)
-        QA_CUDA(qa_launch_fused_open(bt->dev_list, bt->n_models, bt->n, d_Vg, P, a, d_N, d_E, d_xcont, nullptr, d_stats,
+        QA_CUDA(qa_launch_fused_open(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, a, d_N, d_E, d_xcont, nullptr, d_stats,
                                      static_cast<cudaStream_t>(cuda_stream)));
     else
         QA_CUDA(qa_launch_fused_small(bt->dev_list, bt->n_models, bt->n, d_Vg, P, a, d_N, d_E, d_xcont, nullptr, d_stats,

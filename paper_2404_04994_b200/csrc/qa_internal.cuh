@@ -88,8 +88,8 @@ cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const doubl
 cudaError_t qa_launch_fused_small(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
                                   QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
                                   qa_stats *d_stats, cudaStream_t stream);
-cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
-                                 QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
+cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models, int n, int g, const double *d_Vg,
+                                 int64_t P, QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
                                  qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_thermal(const QaDevModel *d_model, int n, QaWorkspace ws, QaCallArgs args, double kT,
                               double expect_cand, double *d_Nmean, double *d_Emin, qa_stats *d_stats, cudaStream_t stream);

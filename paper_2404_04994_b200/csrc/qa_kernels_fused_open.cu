@@ -212,15 +212,48 @@ __device__ __forceinline__ int fo_bucket_rank(int *bucket, int key)
 
 template <int N, bool THR>
 __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDevModel *const *__restrict__ models,
-                                                                   const double *__restrict__ Vg, int64_t P,
+                                                                   const double *__restrict__ Vg, int64_t P, int g,
                                                                    QaCallArgs args, int32_t *__restrict__ outN,
                                                                    double *__restrict__ outE, double *__restrict__ xcont,
                                                                    double *__restrict__ outVs, qa_stats *stats)
 {
     __shared__ __align__(16) FoSmem<N, THR> sm;
-    const QaDevModel *__restrict__ mdl = models[blockIdx.y];
-    const int g = mdl->g;
     const int tid = threadIdx.x;
+    // The thread's two pixels: slot = tid + px * FO_THREADS (coalescing: consecutive threads, consecutive rows).  The first
+    // eight gate voltages of both rows are requested before anything else: their HBM round trip overlaps the staging of the
+    // model tables below (g is a kernel argument so that nothing has to be read to form the addresses).
+    int64_t gp[FO_PX];
+    bool live[FO_PX];
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px) {
+        const int64_t p = (int64_t)blockIdx.x * FO_PIX + px * FO_THREADS + tid;
+        live[px] = p < P;
+        gp[px] = (int64_t)blockIdx.y * P + (live[px] ? p : P - 1);
+    }
+    const double *v0 = Vg + gp[0] * g, *v1 = Vg + gp[1] * g;
+    const bool vec = (g & 1) == 0 && (reinterpret_cast<uintptr_t>(Vg) & 15u) == 0;
+    auto load_chunk = [&](int k0, double (&a)[8], double (&b)[8]) {
+        if (vec) {
+#pragma unroll
+            for (int k = 0; k < 8; k += 2) {
+                double2 ta = make_double2(0.0, 0.0), tb = ta;
+                if (k0 + k < g) {
+                    ta = __ldg(reinterpret_cast<const double2 *>(v0 + k0 + k));
+                    tb = __ldg(reinterpret_cast<const double2 *>(v1 + k0 + k));
+                }
+                a[k] = ta.x, a[k + 1] = ta.y, b[k] = tb.x, b[k + 1] = tb.y;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                a[k] = k0 + k < g ? __ldg(v0 + k0 + k) : 0.0;
+                b[k] = k0 + k < g ? __ldg(v1 + k0 + k) : 0.0;
+            }
+        }
+    };
+    double va[8], vb[8];
+    load_chunk(0, va, vb);
+    const QaDevModel *__restrict__ mdl = models[blockIdx.y];
     for (int e = tid; e < N * N; e += FO_THREADS) {
         sm.MT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
         sm.C[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
@@ -230,53 +263,26 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
     const int ns = mdl->ns;
     __syncthreads();
 
-    // ---- S1-S4 for the thread's two pixels: slot = tid + px * FO_THREADS (coalescing: consecutive threads, consecutive rows)
-    int64_t gp[FO_PX];
-    bool live[FO_PX];
+    // ---- S1-S4
     double nc[FO_PX][N], hp[FO_PX][N];   // hp[b]: energy increment of raising dot N-1-b at the base point
     unsigned freem[FO_PX];               // bit b set: dot N-1-b has two candidate values
     int rounds[FO_PX], rk[FO_PX];
     bool negf[FO_PX], failed[FO_PX], slowf[FO_PX];
 #pragma unroll
-    for (int px = 0; px < FO_PX; ++px) {
-        const int64_t p = (int64_t)blockIdx.x * FO_PIX + px * FO_THREADS + tid;
-        live[px] = p < P;
-        gp[px] = (int64_t)blockIdx.y * P + (live[px] ? p : P - 1);
+    for (int px = 0; px < FO_PX; ++px)
 #pragma unroll
         for (int i = 0; i < N; ++i) nc[px][i] = 0.0;
-    }
-    {   // S1: N_c,i = fma(C_gd[i,k], V[k], acc), k ascending (R1).  Chunks of 8 gates: the 16 loads of a chunk are issued
-        // before its FMAs (the rows come from HBM: one round trip per chunk, not per gate).
-        const double *v0 = Vg + gp[0] * g, *v1 = Vg + gp[1] * g;
-        const bool vec = (g & 1) == 0 && (reinterpret_cast<uintptr_t>(Vg) & 15u) == 0;
-        for (int k0 = 0; k0 < g; k0 += 8) {
-            double a[8], b[8];
-            if (vec) {
+    // S1: N_c,i = fma(C_gd[i,k], V[k], acc), k ascending (R1), in chunks of 8 gates (all loads of a chunk before its FMAs)
+    for (int k0 = 0; k0 < g; k0 += 8) {
+        if (k0 > 0) load_chunk(k0, va, vb);
 #pragma unroll
-                for (int k = 0; k < 8; k += 2) {
-                    double2 ta = make_double2(0.0, 0.0), tb = ta;
-                    if (k0 + k < g) {
-                        ta = __ldg(reinterpret_cast<const double2 *>(v0 + k0 + k));
-                        tb = __ldg(reinterpret_cast<const double2 *>(v1 + k0 + k));
-                    }
-                    a[k] = ta.x, a[k + 1] = ta.y, b[k] = tb.x, b[k + 1] = tb.y;
-                }
-            } else {
+        for (int k = 0; k < 8; ++k) {
+            if (k0 + k < g) {
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    a[k] = k0 + k < g ? __ldg(v0 + k0 + k) : 0.0;
-                    b[k] = k0 + k < g ? __ldg(v1 + k0 + k) : 0.0;
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                if (k0 + k < g) {
-#pragma unroll
-                    for (int i = 0; i < N; ++i) {
-                        const double cg = sm.CgT[(k0 + k) * N + i];
-                        nc[0][i] = fma(cg, a[k], nc[0][i]);
-                        nc[1][i] = fma(cg, b[k], nc[1][i]);
-                    }
+                for (int i = 0; i < N; ++i) {
+                    const double cg = sm.CgT[(k0 + k) * N + i];
+                    nc[0][i] = fma(cg, va[k], nc[0][i]);
+                    nc[1][i] = fma(cg, vb[k], nc[1][i]);
                 }
             }
         }
@@ -551,28 +557,28 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
 }
 
 template <int N>
-cudaError_t launch_fused_open_n(const QaDevModel *const *d_models, int n_models, const double *d_Vg, int64_t P,
+cudaError_t launch_fused_open_n(const QaDevModel *const *d_models, int n_models, const double *d_Vg, int64_t P, int g,
                                 QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
                                 qa_stats *d_stats, cudaStream_t stream)
 {
     const dim3 grid((unsigned)((P + FO_PIX - 1) / FO_PIX), (unsigned)n_models);
     if (args.alg == QA_ALG_DEFAULT)
-        qa_fused_open_kernel<N, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats);
+        qa_fused_open_kernel<N, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont, d_Vs, d_stats);
     else
-        qa_fused_open_kernel<N, true><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats);
+        qa_fused_open_kernel<N, true><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont, d_Vs, d_stats);
     return cudaGetLastError();
 }
 
 }  // namespace
 
 // Open arrays, default or thresholded algorithm, n <= QA_FUSED_MAXN.  Arguments as qa_launch_fused_small.
-cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,
-                                 QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
+cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models, int n, int g, const double *d_Vg,
+                                 int64_t P, QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
                                  qa_stats *d_stats, cudaStream_t stream)
 {
     qa_plan_add("qa_fused_open_kernel");
     if (n_models > 65535 || args.closed || args.alg == QA_ALG_BRUTE_FORCE) return cudaErrorInvalidValue;
-#define CALL(NN) launch_fused_open_n<NN>(d_models, n_models, d_Vg, P, args, d_N, d_E, d_xcont, d_Vs, d_stats, stream)
+#define CALL(NN) launch_fused_open_n<NN>(d_models, n_models, d_Vg, P, g, args, d_N, d_E, d_xcont, d_Vs, d_stats, stream)
     switch (n) {
         case 1: return CALL(1);
         case 2: return CALL(2);
