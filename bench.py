@@ -29,7 +29,9 @@ import numpy as np  # noqa: E402
 METRIC = "candidate configs scored/s (16 dots, default algorithm, open 4x4 grid, 100x100 pixels)"
 UNIT = "candidates/s"
 FP64_OPS_PER_CANDIDATE = 334.0 / 256.0   # FP64-pipe instructions per candidate of the min-plus walk
-WALK_DRAM_BYTES_NCU = 1392384           # profiles/r01_walk_kernel_ncu_full.md: dram__bytes_read + dram__bytes_write per launch
+WALK_DRAM_BYTES_NCU = 1392384           # dram__bytes_read + dram__bytes_write per launch, from the ncu capture named below
+WALK_DRAM_SOURCE = "profiles/r01_walk_kernel_ncu_full.md"
+THERMAL_FP64_OPS_PER_CANDIDATE = {}      # kernel name -> FP64-pipe instructions per weighted candidate
 FP64_LANES_PER_SM = 64         # 148 SMs x 64 FP64 lanes x SM clock
 
 
@@ -39,11 +41,14 @@ def parse():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config4", "config5", "small", "thermal"])
+    ap.add_argument("--workload", default="config4", choices=["config4", "config5", "small", "thermal", "closed16", "sweep"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--arrays", type=int, default=256, help="config5: arrays of the dataset batch per GPU")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--no-parity", action="store_true", help="skip the full-size parity report (profiling runs)")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the secondary workloads of the default run")
+    ap.add_argument("--parity-members", type=int, default=256, help="config-5 members compared with the oracle")
     return ap.parse_args()
 
 
@@ -259,7 +264,9 @@ def run_ours(args, rank, world, local_rank):
     achieved = alg_ops / (walk_ms * 1e-3) if walk_ms > 0 else 0.0
     roofline = {"bound": "alu", "kernel": hot, "achieved": achieved / 1e9, "peak": peak_nominal / 1e9,
                 "unit": "FP64 Ginst/s", "frac": achieved / peak_nominal,
-                "traffic": WALK_DRAM_BYTES_NCU if hot == "qa_minplus_walk_kernel" else None, "traffic_unit": "bytes/launch (ncu dram read+write)",
+                "traffic": WALK_DRAM_BYTES_NCU if hot == "qa_minplus_walk_kernel" else None,
+                "traffic_unit": "bytes/launch (dram__bytes_read.sum + dram__bytes_write.sum)",
+                "traffic_source": "ncu --set full capture of this kernel, " + WALK_DRAM_SOURCE + " (not measured by this run)",
                 "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max_mhz:.0f} MHz "
                                "(DESIGN.md); MEASURED_PEAKS.json has no FP64 figure",
                 "peak_measured_dfma_probe": peak_measured / 1e9, "frac_of_measured_probe": achieved / peak_measured,
@@ -289,6 +296,10 @@ def run_ours(args, rank, world, local_rank):
                "api": "qa_ground_state_host (pinned host buffers)", "n_gpus_measured": 1}
 
     cpu = None if args.no_cpu_baseline else cpu_baseline(args)
+    del flush, Vgs, outs
+    # (N > 1: the other ranks are waiting at the final barrier; the report and the secondary workloads are in the N = 1 line)
+    parity = None if (args.no_parity or world > 1) else parity_report(args)
+    secondary = None if (args.no_secondary or world > 1) else secondary_workloads(args, local_rank)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -302,12 +313,13 @@ def run_ours(args, rank, world, local_rank):
             "ms_per_step_min": float(times.min()), "ms_per_step_median": float(np.median(times)),
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
             "kernels_per_step": plan, "clocks": clocks, "pruned_variant": pruned,
+            "parity": parity, "secondary": secondary,
             "paper_context": "paper: same diagram shape in < 1 s on a GTX 1080 Ti via JAX (PAPER.md L7, L498)"}
     print(json.dumps(line), flush=True)
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-def run_config5(args, rank, world, local_rank):
+def run_config5(args, rank, world, local_rank, steps=None, emit=True):
     """Secondary workload (BASELINE.json configs[4]): the dataset batch of independently seeded open 8-dot arrays, each a
     128x128 sweep, with the default algorithm and the thresholded one at t = 0.2 and 0.5.  One step = every array with
     all three algorithms, through qa_ground_state_batch (semantically a loop over the single-model call, one launch of
@@ -317,6 +329,7 @@ def run_config5(args, rank, world, local_rank):
     import torch.distributed as dist
     from paper_2404_04994_b200 import api, workloads as wl
 
+    steps = steps or args.steps
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     B = args.arrays
@@ -348,8 +361,8 @@ def run_config5(args, rank, world, local_rank):
     sampler = ClockSampler(local_rank)
     sampler.start()
     barrier()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for k in range(args.steps):
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for k in range(steps):
         flush.fill_(k & 0xff)
         ev[k][0].record()
         step()
@@ -362,9 +375,9 @@ def run_config5(args, rank, world, local_rank):
         tt = torch.tensor([tot_ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         tot_ms = float(tt.item())
-    ms_per_step = tot_ms / args.steps
+    ms_per_step = tot_ms / steps
     if rank != 0:
-        return
+        return None
     agree = {}
     for a in ("t0.2", "t0.5"):
         same = int((outs[a]["N"] == outs["default"]["N"]).all(dim=2).sum())
@@ -379,7 +392,7 @@ def run_config5(args, rank, world, local_rank):
     peak = hbm or 6516.0
     achieved = px_step * bytes_px / (ms_per_step * 1e-3) / 1e9
     line = {"metric": "pixels/s over the dataset batch (open 8-dot arrays, 128x128, default + thresholded t=0.2, 0.5)",
-            "value": world * px_step / (ms_per_step * 1e-3), "unit": "pixels/s", "n_gpus": world, "steps": args.steps,
+            "value": world * px_step / (ms_per_step * 1e-3), "unit": "pixels/s", "n_gpus": world, "steps": steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[4]: {B} open 8-dot arrays (seeds 1000+j), 128x128 each, "
@@ -390,18 +403,24 @@ def run_config5(args, rank, world, local_rank):
             "agreement_with_default": agree,
             "roofline": {"bound": "hbm", "kernel": "qa_fused_small_kernel (whole step: 3 launches)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                         "bytes_per_pixel": bytes_px,
+                         "bytes_per_pixel": bytes_px, "algorithmic_bytes_per_step": px_step * bytes_px,
+                         "traffic_source": "not measured by this run; ncu figure in profiles/r02_config5_ncu.md",
                          "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm else "fallback 6516 GB/s (SURVEY.md)"},
-            "cpu_baseline": None, "e2e": None, "gpu_launches": launches_per_step * args.steps, "clocks": clocks}
-    print(json.dumps(line), flush=True)
+            "cpu_baseline": None, "e2e": None, "gpu_launches": launches_per_step * steps, "clocks": clocks}
+    line["ms_per_step_median"] = float(np.median(times))
+    del Vg, outs, flush
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-def run_small(args, rank):
+def run_small(args, rank, steps=None, emit=True):
     """BASELINE.json configs[0..2] (launch-latency-bound diagrams: 10^4 - 4*10^4 pixels, <= 7776 candidates per pixel):
     device time of one diagram per (config, algorithm), CUDA events, L2 flushed between repetitions.  One JSON line."""
     if rank != 0:
-        return
+        return None
+    steps = steps or args.steps
     import torch
     from paper_2404_04994_b200 import api, workloads as wl
     dev = torch.device("cuda", 0)
@@ -417,8 +436,8 @@ def run_small(args, rank):
         for kw in kws:
             for _ in range(max(3, args.warmup)):
                 m.ground_state(Vg, regime=w.regime, N_hat=w.N_hat, **kw)
-            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-            for k in range(args.steps):
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+            for k in range(steps):
                 flush.fill_(k & 0xff)
                 ev[k][0].record()
                 r = m.ground_state(Vg, regime=w.regime, N_hat=w.N_hat, want_stats=(k == 0), **kw)
@@ -432,18 +451,41 @@ def run_small(args, rank):
                          "ms_min": float(t.min()), "pixels_per_s": w.P / (float(np.median(t)) * 1e-3),
                          "candidates_enumerated": sd["n_candidates_enumerated"], "candidates_scored": sd["n_candidates_scored"],
                          "qp_pixels": sd["n_qp_pixels"], "kernels": api.last_launch_plan()[0]})
-    print(json.dumps({"metric": "device time per diagram, BASELINE.json configs[0..2]", "unit": "ms", "n_gpus": 1,
-                      "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
-                      "l2": "flushed (256 MiB write) between repetitions", "rows": rows}), flush=True)
+    line = {"metric": "device time per diagram, BASELINE.json configs[0..2]", "unit": "ms", "n_gpus": 1,
+            "steps": steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
+            "l2": "flushed (256 MiB write) between repetitions", "rows": rows}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-def run_thermal(args, rank):
+def _time_calls(torch, fn, steps, warmup, flush):
+    """Median / min / mean device time (ms) of fn() over `steps` repetitions, CUDA events, L2 flushed in between."""
+    for _ in range(max(3, warmup)):
+        fn()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for k in range(steps):
+        flush.fill_(k & 0xff)
+        ev[k][0].record()
+        fn()
+        ev[k][1].record()
+    torch.cuda.synchronize()
+    t = np.array([a.elapsed_time(b) for a, b in ev])
+    return float(np.median(t)), float(t.min()), float(t.mean())
+
+
+def _fp64_peak(torch, dev=0):
+    return torch.cuda.get_device_properties(dev).multi_processor_count * FP64_LANES_PER_SM * 1965.0e6
+
+
+def run_thermal(args, rank, steps=None, emit=True):
     """thermal broadening (Eq. (10)) on the config-4 diagram (16 dots, 100x100, default set: 2^16
     Boltzmann weights per pixel), kT = 0.05 E_C.  Device time per diagram (CUDA events, L2 flushed) and the oracle on one
     host core on a bounded sample.  One JSON line."""
     if rank != 0:
-        return
+        return None
+    steps = steps or args.steps
     import torch
     import oracle
     from paper_2404_04994_b200 import api, workloads as wl
@@ -455,37 +497,185 @@ def run_thermal(args, rank):
     kT = 0.05 * EC
     Vg = torch.from_numpy(w.Vg).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    for _ in range(max(3, args.warmup)):
-        m.thermal(Vg, kT)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for k in range(args.steps):
-        flush.fill_(k & 0xff)
-        ev[k][0].record()
-        r = m.thermal(Vg, kT)
-        ev[k][1].record()
+    ms, ms_min, _ = _time_calls(torch, lambda: m.thermal(Vg, kT), steps, args.warmup, flush)
+    r = m.thermal(Vg, kT)
+    plan = api.last_launch_plan()[0]
+    kt = api.kernel_times(m, Vg, steps=min(steps, 5), flush=flush, call="thermal", kT=kT)
     torch.cuda.synchronize()
-    t = np.array([a.elapsed_time(b) for a, b in ev])
-    kt = api.kernel_times(m, Vg, steps=5, flush=flush) if False else None
     om = oracle.Model(w.C_dd, w.C_gd)
     sel = np.sort(np.random.default_rng(0).choice(w.P, size=40, replace=False))
     t0 = time.perf_counter()
     o = om.thermal(w.Vg[sel], kT)
     dt = time.perf_counter() - t0
     err = float(np.abs(r["Nmean"].cpu().numpy()[sel] - o["Nmean"]).max())
-    ms = float(np.median(t))
-    print(json.dumps({"metric": "Boltzmann-weighted candidate configs/s (thermal broadening, 16 dots, default set, 100x100)",
-                      "value": w.P * 65536 / (ms * 1e-3), "unit": "candidates/s", "n_gpus": 1, "steps": args.steps,
-                      "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_min": float(t.min()), "higher_is_better": True,
-                      "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": "BASELINE.json configs[3] with Eq. (10), kT = 0.05 E_C", "kT": kT,
-                                 "l2": "flushed (256 MiB write) between timed steps"},
-                      "kernels_per_step": api.last_launch_plan()[0], "max_abs_err_vs_oracle_sample": err,
-                      "cpu_baseline": {"value": len(sel) * 65536 / dt, "unit": "candidates/s", "cores": 1, "kind": "oracle",
-                                       "sample": f"{len(sel)} of 10000 pixels (seeded random subset), {dt:.1f} s"}}), flush=True)
+    hot = max(kt, key=kt.get) if kt else None
+    ops = THERMAL_FP64_OPS_PER_CANDIDATE.get(hot.split("<")[0], None) if hot else None
+    roof = None
+    if ops:
+        ach = ops * w.P * 65536 / (kt[hot] * 1e-3)
+        roof = {"bound": "alu", "kernel": hot, "achieved": ach / 1e9, "peak": _fp64_peak(torch) / 1e9, "unit": "FP64 Ginst/s",
+                "frac": ach / _fp64_peak(torch), "fp64_ops_per_candidate": ops, "kernel_ms": kt[hot], "kernel_times_ms": kt,
+                "traffic": None, "peak_source": "derived: SMs x 64 FP64 lanes x 1965 MHz (DESIGN.md section 6)"}
+    line = {"metric": "Boltzmann-weighted candidate configs/s (thermal broadening, 16 dots, default set, 100x100)",
+            "value": w.P * 65536 / (ms * 1e-3), "unit": "candidates/s", "n_gpus": 1, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_min": ms_min, "higher_is_better": True,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[3] with Eq. (10), kT = 0.05 E_C", "kT": kT,
+                       "l2": "flushed (256 MiB write) between timed steps"},
+            "kernels_per_step": plan, "roofline": roof, "max_abs_err_vs_oracle_sample": err,
+            "cpu_baseline": {"value": len(sel) * 65536 / dt, "unit": "candidates/s", "cores": 1, "kind": "oracle",
+                             "sample": f"{len(sel)} of 10000 pixels (seeded random subset), {dt:.1f} s"}}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def run_closed16(args, rank, steps=None, emit=True):
+    """SURVEY 8(f) NEXT-3, the paper's second headline shape (Fig. 4(b)): CLOSED array of 16 dots with
+    N_hat = n_dot = 16, default algorithm, 100x100 pixels, on the config-4 model and sweep.  Only the C(16, k) floor/ceil
+    states with the right total are scored (k = N_hat - sum floor(x) per pixel).  Reports candidates SCORED/s, the time
+    per diagram, and every pixel against the oracle (OpenMP)."""
+    if rank != 0:
+        return None
+    steps = steps or args.steps
+    import torch
+    import oracle
+    from paper_2404_04994_b200 import api, workloads as wl
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from parity import compare
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    w = wl.config4(100, 100)
+    n = w.n_dot
+    m = api.Model(w.C_dd, w.C_gd)
+    Vg = torch.from_numpy(w.Vg).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    kw = dict(regime="closed", N_hat=n)
+    ms, ms_min, _ = _time_calls(torch, lambda: m.ground_state(Vg, **kw), steps, args.warmup, flush)
+    r = m.ground_state(Vg, want_xcont=True, want_stats=True, **kw)
+    plan = api.last_launch_plan()[0]
+    kt = api.kernel_times(m, Vg, steps=min(steps, 10), flush=flush, **kw)
+    torch.cuda.synchronize()
+    st = api.stats_dict(r["stats"])
+    om = oracle.Model(w.C_dd, w.C_gd)
+    t0 = time.perf_counter()
+    o = om.ground_state(w.Vg, n_threads=os.cpu_count(), **kw)
+    dt = time.perf_counter() - t0
+    rep = compare(r["N"].cpu().numpy(), r["E"].cpu().numpy(), o, om.EC, gpu_x=r["xcont"].cpu().numpy(), strict=False)
+    # the generic odometer (all 2^16 states visited, filtered on the total) on the same diagram, for reference
+    m0 = api.Model(w.C_dd, w.C_gd, walk_variant=0)
+    ms0, _, _ = _time_calls(torch, lambda: m0.ground_state(Vg, **kw), max(3, steps // 4), 3, flush)
+    hot = max(kt, key=kt.get) if kt else None
+    line = {"metric": "candidate configs scored/s (closed array, 16 dots, N_hat = 16, default algorithm, 100x100 pixels)",
+            "value": st["n_candidates_scored"] / (ms * 1e-3), "unit": "candidates/s", "n_gpus": 1, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_min": ms_min, "higher_is_better": True, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[3] model and sweep, closed with N_hat = 16 (PAPER.md L496)",
+                       "l2": "flushed (256 MiB write) between timed steps"},
+            "pixels_per_s": w.P / (ms * 1e-3), "candidates_scored_per_step": st["n_candidates_scored"],
+            "candidates_enumerated_per_step": st["n_candidates_enumerated"], "qp_pixels": st["n_qp_pixels"],
+            "kernels_per_step": plan, "kernel_times_ms": kt, "hot_kernel": hot,
+            "generic_odometer_ms_per_step": ms0, "speedup_over_generic_odometer": ms0 / ms,
+            "parity": rep,
+            "cpu_baseline": {"value": int(o["n_scored"].sum()) / dt, "unit": "candidates/s", "cores": os.cpu_count(),
+                             "kind": "oracle", "sample": f"the whole diagram, OpenMP over pixels, {dt:.1f} s"},
+            "paper_context": "paper: closed 16-dot 100x100 diagram in < 1 s (PAPER.md L7, L498)"}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def run_sweep(args, rank, steps=None, emit=True):
+    """the SHAPE of the paper's Fig. 4(a)/(b): device time of a 100x100 diagram
+    of a random Maxwell array for n_dot = 2..16, default algorithm, open and closed (N_hat = n_dot), random C and V_g as
+    L490, with the oracle's time per pixel (one core, bounded sample) beside it."""
+    if rank != 0:
+        return None
+    steps = steps or args.steps
+    import torch
+    import oracle
+    from paper_2404_04994_b200 import api, workloads as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    rows = []
+    for n in range(2, 17):
+        w = wl.random_open(n, n, 10000, seed=4000 + n, lo=-0.3, hi=2.5)
+        m = api.Model(w.C_dd, w.C_gd)
+        Vg = torch.from_numpy(w.Vg).to(dev)
+        om = oracle.Model(w.C_dd, w.C_gd)
+        px = max(4, min(2000, int(2.0e6 / (2 ** n))))
+        row = {"n_dot": n}
+        for regime, kw in (("open", dict()), ("closed", dict(regime="closed", N_hat=n))):
+            med, mn, _ = _time_calls(torch, lambda: m.ground_state(Vg, **kw), steps, 3, flush)
+            plan = api.last_launch_plan()[0]
+            t0 = time.perf_counter()
+            om.ground_state(w.Vg[:px], **kw)
+            dt = (time.perf_counter() - t0) / px
+            row[regime] = {"ms_per_diagram": med, "ms_min": mn, "kernels": plan,
+                           "oracle_ms_per_diagram_1core_extrapolated": dt * 1e4 * 1e3, "oracle_sample_pixels": px}
+        rows.append(row)
+    line = {"metric": "device time of a 100x100 diagram vs n_dot (default algorithm; shape of PAPER.md Fig. 4)",
+            "unit": "ms", "n_gpus": 1, "steps": steps, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "random dense Maxwell arrays (workloads.random_open, seeds 4000+n), 10^4 random gate "
+                                   "vectors, open and closed with N_hat = n_dot (PAPER.md L490, L496)",
+                       "l2": "flushed (256 MiB write) between repetitions"},
+            "rows": rows}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def parity_report(args):
+    """Every pixel of the five BASELINE.json configs at full size, CUDA path through the binding vs the oracle (OpenMP
+    over the host cores); run AFTER the timed region.  tests/parity.py holds the rule (north_star: bit-exact except
+    near-ties of the oracle below 1e-9 E_C, counted)."""
+    import torch
+    import oracle
+    from paper_2404_04994_b200 import api, workloads as wl
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from parity import full_size_report
+    t0 = time.perf_counter()
+    rep = full_size_report(api, oracle, wl, torch, strict=False, config5_members=args.parity_members)
+    rep["wall_s"] = round(time.perf_counter() - t0, 1)
+    rep["oracle_threads"] = os.cpu_count()
+    rep["unexcused_total"] = int(sum(v.get("unexcused", 0) + v.get("sensor_unexcused", 0) + v.get("unexcused_all_variants", 0)
+                                     for v in rep.values() if isinstance(v, dict)))
+    rep["rule"] = ("N bit-exact except pixels whose oracle best/second-best energies differ by < 1e-9 E_C (counted as "
+                   "excused_near_tie); |dE| <= 1e-9 max(|E|, E_C); |dx| <= 1e-9 max(1, |x|), bit-identical without QP")
+    return rep
+
+
+def secondary_workloads(args, local_rank):
+    """The other workloads, measured in the same (default) run so that the driver observes them: the dataset batch
+    (config 5), the small configs 1-3, the closed 16-dot diagram, thermal broadening and the n_dot sweep."""
+    out = {}
+    for name, fn in (("config5", lambda: run_config5(args, 0, 1, local_rank, steps=10, emit=False)),
+                     ("small", lambda: run_small(args, 0, steps=12, emit=False)),
+                     ("closed16", lambda: run_closed16(args, 0, steps=12, emit=False)),
+                     ("thermal", lambda: run_thermal(args, 0, steps=5, emit=False)),
+                     ("sweep", lambda: run_sweep(args, 0, steps=5, emit=False))):
+        try:
+            out[name] = fn()
+        except Exception as e:  # a secondary workload must never cost the headline line
+            out[name] = {"error": f"{type(e).__name__}: {e}"}
+    return out
 
 
 def main():
     args = parse()
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # `python bench.py --gpus N` launched plainly: start one rank per GPU ourselves (the driver's torchrun command line)
+        port = 29500 + (os.getpid() % 2000)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")          # the communicator log shows the ranks
+        env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        raise SystemExit(subprocess.call(cmd, env=env))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -505,6 +695,10 @@ def main():
         run_thermal(args, rank)
     elif args.workload == "small":
         run_small(args, rank)
+    elif args.workload == "closed16":
+        run_closed16(args, rank)
+    elif args.workload == "sweep":
+        run_sweep(args, rank)
     elif args.workload == "config5":
         run_config5(args, rank, world, local_rank)
     else:

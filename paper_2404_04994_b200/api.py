@@ -342,16 +342,18 @@ def measure_fp64_rate(seconds: float = 1.0) -> float:
     return r.value
 
 
-def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch.Tensor | None = None, **kw) -> dict:
-    """Average device time (ms) of each kernel of model.ground_state(Vg, **kw), from CUDA events recorded by the library
-    between its kernels on the launching stream (qa_set_kernel_timing / qa_get_kernel_timings)."""
+def kernel_times(model: "Model", Vg: torch.Tensor, steps: int = 10, flush: torch.Tensor | None = None, call: str = "ground_state",
+                 **kw) -> dict:
+    """Average device time (ms) of each kernel of model.ground_state(Vg, **kw) (or model.thermal with call="thermal"), from
+    CUDA events recorded by the library between its kernels on the launching stream (qa_set_kernel_timing /
+    qa_get_kernel_timings)."""
     acc: dict = {}
     lib().qa_set_kernel_timing(1)
     try:
         for k in range(steps):
             if flush is not None:
                 flush.fill_(k & 0xff)
-            model.ground_state(Vg, **kw)
+            getattr(model, call)(Vg, **kw)
             ms = (C.c_float * 8)()
             n = C.c_int()
             _check(lib().qa_get_kernel_timings(8, ms, C.byref(n)), "qa_get_kernel_timings")

@@ -284,6 +284,10 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
                                        variant == 2, stream));
         timing_mark(stream);
         if (fuse) return QA_OK;
+    } else if (alg == QA_ALG_DEFAULT && closed && n > QA_WALK_NL && variant != 0) {
+        // closed default set of a larger array: only the C(n, k) states with the right total are visited (NEXT-3)
+        QA_CUDA(qa_launch_closed_walk(m->dev, n, m->walk, ws, a, d_stats, m->sm_count, stream));
+        timing_mark(stream);
     } else if (alg == QA_ALG_DEFAULT && !closed) {
         QA_CUDA(qa_launch_walk(m->dev, n, m->walk, ws, d_stats, m->sm_count, stream));
         timing_mark(stream);

@@ -83,6 +83,8 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
                                 qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, qa_stats *d_stats,
                            int sm_count, cudaStream_t stream);
+cudaError_t qa_launch_closed_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, QaCallArgs args,
+                                  qa_stats *d_stats, int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
                                    double *d_E, int sm_count, int pruned, cudaStream_t stream);
 cudaError_t qa_launch_fused_small(const QaDevModel *const *d_models, int n_models, int n, const double *d_Vg, int64_t P,

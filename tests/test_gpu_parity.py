@@ -242,6 +242,39 @@ def test_all_sizes_closed_and_thresholded(api, n, variant):
         check(api, w, variant=variant, algorithm="brute", n_max=3)
 
 
+# ---- closed arrays at scale: only the C(n, k) states with the right total are visited ------------
+@pytest.mark.parametrize("n", list(range(9, 17)))
+def test_closed_default_large_arrays(api, n):
+    """Closed default search for n = 9..16 through qa_closed_walk_kernel (popcount classes of the min-plus split), N_hat = n
+     and a second total, QP pixels included, element by element against the oracle; the scored-candidate
+    counter must equal the oracle's sum of C(n, N_hat - sum lo).  Variant 0 (the generic odometer over all 2^n states,
+    filtered) must give the same maps.  Also a general SPD c_dd (no Maxwell structure is used by the kernel)."""
+    P = 301 if n <= 12 else (131 if n <= 14 else 67)
+    for N_hat in (n, max(1, n // 3)):
+        w = wl.random_open(n, n, P, seed=700 + n, lo=-0.5, hi=2.4)
+        w.regime, w.N_hat = "closed", N_hat
+        rep, g, o = check(api, w, algorithm="default")
+        assert g["plan"][0] == ["qa_prologue_kernel", "qa_closed_walk_kernel", "qa_finalize_kernel"]
+        assert g["stats"]["n_qp_pixels"] > 0
+        rep0, g0, _ = check(api, w, variant=0, algorithm="default")
+        assert g0["plan"][0][1].startswith("qa_enumerate_kernel")
+        assert np.array_equal(g["N"], g0["N"])
+    w = wl.random_general(n, n, 61, seed=740 + n)
+    w.regime, w.N_hat = "closed", n
+    rep, g, o = check(api, w, algorithm="default")
+    assert g["plan"][0][1] == "qa_closed_walk_kernel"
+
+
+def test_closed_default_edge_totals(api):
+    """N_hat = 0 (only the all-zero state), N_hat far above what the gates ask for, and P not a multiple of the pixels per
+    CTA, on a 10-dot and a 16-dot array."""
+    for n, P in ((10, 97), (16, 13)):
+        for N_hat in (0, 1, 3 * n):
+            w = wl.random_open(n, n, P, seed=760 + n, lo=-0.5, hi=2.4)
+            w.regime, w.N_hat = "closed", N_hat
+            check(api, w, algorithm="default")
+
+
 # ---- c_dd with positive off-diagonals (SPD, not Maxwell): general active-set phase of the QP (reading R3) -------------
 @pytest.mark.parametrize("n", [2, 3, 5, 8, 11, 13, 16])
 def test_general_spd_matrices(api, n):

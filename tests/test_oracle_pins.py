@@ -348,6 +348,21 @@ def test_P10_candidate_counts():
     assert np.array_equal(rcd["n_scored"], [comb(5, int(v)) for v in k])
 
 
+def test_P10_closed_default_scores_C_n_k_states_at_16_dots():
+    """Closed default set at n = 16, N_hat = 16 (Fig. 4(b) shape, L496): 2^16 enumerated, exactly C(16, N_hat - sum lo) scored
+    (L127: candidates with the wrong total are eliminated) -- 12 870 when k = 8 -- and the winner carries the total."""
+    from math import comb
+    from paper_2404_04994_b200 import workloads as wl
+    w = wl.config4(5, 4)
+    m = oracle.Model(w.C_dd, w.C_gd)
+    r = m.ground_state(w.Vg, regime="closed", N_hat=16)
+    lo = np.maximum(np.floor(r["x"]), 0).astype(int)
+    k = 16 - lo.sum(1)
+    assert (r["n_enum"] == 65536).all() and (k >= 0).all() and (k <= 16).all()
+    assert np.array_equal(r["n_scored"], [comb(16, int(v)) for v in k])
+    assert (r["N"].sum(1) == 16).all() and ((r["N"] - lo) >= 0).all() and ((r["N"] - lo) <= 1).all()
+
+
 # ---------------------------------------------------------------------------------------------------------- P11
 def _qp_by_active_set_enumeration(M, c, closed, N_hat):
     """All 2^n active sets with numpy; returns the unique KKT point (strict convexity, App. B)."""
