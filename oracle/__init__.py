@@ -39,6 +39,12 @@ def _lib(omp: bool = False):
                                    lp, ip]
         lib.qo_sensor.argtypes = [vp, vp, ip, C.c_int, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip,
                                   dp, dp, dp, dp, ip]
+        lib.qo_rng_u64.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64]
+        lib.qo_rng_u64.restype = C.c_uint64
+        for f in ("qo_rng_uniform", "qo_rng_normal"):
+            getattr(lib, f).argtypes = [C.c_uint64, C.c_uint64, C.c_uint64]
+            getattr(lib, f).restype = C.c_double
+        lib.qo_sensor_response.argtypes = [dp, C.c_int64, C.c_int, C.c_int64, vp, dp, dp]
         _libs[key] = lib
     return _libs[key]
 
@@ -179,6 +185,50 @@ def sensor_ground_state(C_dd, C_gd, sensor_dots, Vg, regime="open", N_hat=0, alg
     if rc:
         raise ValueError(f"qo_sensor: invalid argument ({rc})")
     return out
+
+
+class SensorParams(C.Structure):
+    """Parameters of one sensor's response (reading R14; mirrors qo_sensor_params)."""
+    _fields_ = [("profile", C.c_int32), ("pink_octaves", C.c_int32), ("v0", C.c_double), ("width", C.c_double),
+                ("amplitude", C.c_double), ("white_sigma", C.c_double), ("pink_sigma", C.c_double),
+                ("jump_rate", C.c_double), ("jump_sigma", C.c_double), ("seed", C.c_uint64)]
+
+
+PROFILE = {"lorentzian": 0, "gaussian": 1, "linear": 2}
+
+
+def sensor_params(profile="lorentzian", v0=0.0, width=1.0, amplitude=1.0, white_sigma=0.0, pink_sigma=0.0, pink_octaves=0,
+                  jump_rate=0.0, jump_sigma=0.0, seed=0):
+    return SensorParams(PROFILE[profile] if isinstance(profile, str) else int(profile), int(pink_octaves), float(v0),
+                        float(width), float(amplitude), float(white_sigma), float(pink_sigma), float(jump_rate),
+                        float(jump_sigma), int(seed))
+
+
+def sensor_response(Vs, W, params, want_gradient=True):
+    """Reading R14 (L149, L464): response profile + white / 1/f / jump noise of every sensor column of Vs[P, ns], and its
+    gradient along the fast axis (row length W).  params: one SensorParams per sensor.  Returns dict(S[, G])."""
+    Vs = np.ascontiguousarray(Vs, dtype=np.float64)
+    Vs = Vs.reshape(Vs.shape[0], -1)
+    P, ns = Vs.shape
+    arr = (SensorParams * ns)(*params)
+    S = np.empty((P, ns))
+    G = np.empty((P, ns)) if want_gradient else None
+    rc = _lib().qo_sensor_response(_dp(Vs), P, ns, int(W), C.byref(arr), _dp(S), _dp(G))
+    if rc:
+        raise ValueError(f"qo_sensor_response: invalid argument ({rc})")
+    return dict(S=S, G=G) if want_gradient else dict(S=S)
+
+
+def rng_u64(seed, stream, idx):
+    return int(_lib().qo_rng_u64(seed, stream, idx))
+
+
+def rng_uniform(seed, stream, idx):
+    return float(_lib().qo_rng_uniform(seed, stream, idx))
+
+
+def rng_normal(seed, stream, idx):
+    return float(_lib().qo_rng_normal(seed, stream, idx))
 
 
 def has_openmp() -> bool:

@@ -20,12 +20,16 @@
  *   5. argmin (Eq. (5)), ties -> lexicographically smallest N (reading R6); also the second-best energy
  *   6. charge-sensor dots (L149, Eq. (3); reading R8)
  *   7. thermal broadening: the soft arg min of Eq. (10) L157 over the same candidate set (qo_thermal; reading R13)
+ *   8. charge-sensor response profile, noise and gradient (qo_sensor_response; L149, L464; reading R14)
  *
  * Pins (tests/test_oracle_*.py): P0..P13 of DESIGN.md (P13: Eq. (10) -- Fermi function of a single dot, kT -> 0 and
  * kT -> infinity limits, Eq. (4)-energy numpy sums on tiny arrays, sum <N> = N_hat).  Functions with no pin independent of the oracle itself:
  *   - qo_sensor's potential values on random arrays                           : "parity unpinned" beyond the
  *     single-sensor closed form tested in tests/test_oracle_pins.py (rounding of s, V_s = [M (N - N_c)]_s)
  *   - thresholded-vs-default agreement RATE on config 5                       : parity unpinned (statistic only)
+ *   - qo_sensor_response: the paper gives neither formula nor parameter for the response profile and the noise
+ *     (L149), so WHICH profile / noise model is right is "parity unpinned"; what reading R14 fixes is pinned (profile
+ *     closed forms, SplitMix64 test vector, moments / spectrum / jump statistics of the noise, numpy.gradient)
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fPIC -shared [-fopenmp]   (oracle/build.py).
  */
@@ -633,6 +637,106 @@ int qo_sensor(const qo_model *full, const qo_model *sub, const int32_t *sensor_i
             for (int j = 0; j < n; j++) v += full->M[s * n + j] * d[j];
             Vs[p * ns + a] = v;
         }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------------ */
+/* 8. charge-sensor RESPONSE and noise (L149 last two sentences; reading R14 of DESIGN.md).        */
+/* The paper names the ingredients but prints no formula or parameter ("Lorentzian or an approximately Gaussian        */
+/* profile in the weak and strong coupling regimes"; "white, 1/f, and sensor jump noise can be added on top"; Fig. 3   */
+/* L464 plots the derivative of the sensor signal along the swept gate and, for a qpc, "replaced the Lorentzian shape  */
+/* response with a linear function").  Reading R14 fixes every choice; all parameters are the caller's.                */
+/*   profile 0 Lorentzian  S = A / (1 + ((V_s - v0)/w)^2)          w = half width at half maximum                       */
+/*   profile 1 Gaussian    S = A exp(-(V_s - v0)^2 / (2 w^2))      w = standard deviation                               */
+/*   profile 2 linear      S = A (V_s - v0) / w                    (qpc, L464)                                          */
+/* Noise is added to S in pixel order p = iy W + ix (the raster is the time axis):                                      */
+/*   white   sigma_w z(0, p)                                                                                           */
+/*   1/f     (sigma_p / sqrt K) sum_{j<K} z(1 + j, p >> j)    Voss-McCartney: source j is redrawn every 2^j pixels      */
+/*   jumps   J(p) = sum_{q<=p} [u(62, q) < rate] sigma_j z(31, q)   the baseline keeps every shift (sequential sum)     */
+/* Random numbers are counter based (so that any implementation draws the same ones in any order):                     */
+/*   r(stream, idx) = mix(mix(seed + GOLDEN (stream + 1)) + GOLDEN (idx + 1)),  mix = the SplitMix64 finaliser          */
+/*   u = ((r >> 11) + 0.5) 2^-53 in (0,1);  z(s, idx) = sqrt(-2 ln u(2s, idx)) cos(2 pi u(2s + 1, idx))  (Box-Muller)   */
+/*   sensor a uses the streams 128 a + (...).                                                                          */
+/* Gradient (optional): along the fast axis ix, central differences inside a row, one-sided at its two ends, in signal */
+/* units per pixel; taken of the noisy signal.                                                                         */
+typedef struct {
+    int32_t profile;       /* 0 Lorentzian, 1 Gaussian, 2 linear */
+    int32_t pink_octaves;  /* K, 0..30 */
+    double v0, width, amplitude;
+    double white_sigma, pink_sigma, jump_rate, jump_sigma;
+    uint64_t seed;
+} qo_sensor_params;
+
+#define QO_GOLDEN 0x9E3779B97F4A7C15ull
+static uint64_t qo_mix64(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+uint64_t qo_rng_u64(uint64_t seed, uint64_t stream, uint64_t idx)
+{
+    return qo_mix64(qo_mix64(seed + QO_GOLDEN * (stream + 1)) + QO_GOLDEN * (idx + 1));
+}
+double qo_rng_uniform(uint64_t seed, uint64_t stream, uint64_t idx)
+{
+    return ((double)(qo_rng_u64(seed, stream, idx) >> 11) + 0.5) * 0x1.0p-53;
+}
+double qo_rng_normal(uint64_t seed, uint64_t stream, uint64_t idx)
+{
+    double u1 = qo_rng_uniform(seed, 2 * stream, idx), u2 = qo_rng_uniform(seed, 2 * stream + 1, idx);
+    return sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925286766559 * u2);
+}
+
+double qo_sensor_profile(const qo_sensor_params *q, double vs)
+{
+    double x = (vs - q->v0) / q->width;
+    if (q->profile == 0) return q->amplitude / (1.0 + x * x);
+    if (q->profile == 1) return q->amplitude * exp(-0.5 * x * x);
+    return q->amplitude * x;
+}
+
+int qo_sensor_response(const double *Vs /* [P][ns] */, int64_t P, int ns, int64_t W, const qo_sensor_params *prm /* [ns] */,
+                       double *S /* [P][ns] */, double *G /* [P][ns] or NULL */)
+{
+    if (P < 0 || ns < 1 || W < 1 || (P % W) != 0) return 1;
+    for (int a = 0; a < ns; a++) {
+        const qo_sensor_params *q = prm + a;
+        if (q->profile < 0 || q->profile > 2 || !(q->width > 0.0) || q->pink_octaves < 0 || q->pink_octaves > 30 ||
+            q->white_sigma < 0.0 || q->pink_sigma < 0.0 || q->jump_sigma < 0.0 || !(q->jump_rate >= 0.0 && q->jump_rate <= 1.0))
+            return 1;
+        uint64_t st = 128ull * (uint64_t)a;
+        double J = 0.0;
+        for (int64_t p = 0; p < P; p++) {
+            double s = qo_sensor_profile(q, Vs[p * ns + a]);
+            if (q->white_sigma > 0.0) s += q->white_sigma * qo_rng_normal(q->seed, st + 0, (uint64_t)p);
+            if (q->pink_sigma > 0.0 && q->pink_octaves > 0) {
+                double acc = 0.0;
+                for (int j = 0; j < q->pink_octaves; j++) acc += qo_rng_normal(q->seed, st + 1 + (uint64_t)j, (uint64_t)p >> j);
+                s += q->pink_sigma / sqrt((double)q->pink_octaves) * acc;
+            }
+            if (q->jump_rate > 0.0 && q->jump_sigma > 0.0) {
+                if (qo_rng_uniform(q->seed, 2 * (st + 62), (uint64_t)p) < q->jump_rate)
+                    J += q->jump_sigma * qo_rng_normal(q->seed, st + 31, (uint64_t)p);
+                s += J;
+            }
+            S[p * ns + a] = s;
+        }
+    }
+    if (G) {
+        int64_t H = P / W;
+        for (int64_t iy = 0; iy < H; iy++)
+            for (int64_t ix = 0; ix < W; ix++)
+                for (int a = 0; a < ns; a++) {
+                    const double *row = S + iy * W * ns + a;
+                    double g;
+                    if (W == 1) g = 0.0;
+                    else if (ix == 0) g = row[ns] - row[0];
+                    else if (ix == W - 1) g = row[(W - 1) * ns] - row[(W - 2) * ns];
+                    else g = 0.5 * (row[(ix + 1) * ns] - row[(ix - 1) * ns]);
+                    G[(iy * W + ix) * ns + a] = g;
+                }
     }
     return 0;
 }

@@ -727,3 +727,111 @@ def test_P13_brute_force_box_and_bounds():
     assert (o["Nmean"] >= 0).all() and (o["Nmean"] <= 3).all()
     with pytest.raises(ValueError):
         m.thermal(Vg, 0.0)
+
+
+# ---------------------------------------------------------------------------------------------------------- P14
+# Sensor response, noise and gradient (L149, L464; reading R14).  The paper prints no formula: what is pinned is what R14 fixes.
+def test_P14_response_profiles_closed_forms():
+    """Lorentzian: S(v0) = A, S(v0 +- w) = A/2 (w = HWHM), symmetric, S(v0 + 3w) = A/10; Gaussian: S(v0 +- w) = A e^-1/2,
+    inflection at +-w; linear: A (V - v0)/w; Lorentzian and Gaussian agree to second order at the peak after matching
+    curvature (w_G = w_L / sqrt 2)."""
+    A, v0, w = 2.5, 0.3, 0.07
+    V = np.array([v0, v0 + w, v0 - w, v0 + 3 * w, v0 - 3 * w, v0 + 1e-4, v0 - 1e-4])[:, None]
+    L = oracle.sensor_response(V, 1, [oracle.sensor_params("lorentzian", v0, w, A)])["S"][:, 0]
+    assert L[0] == A and abs(L[1] - A / 2) < 1e-15 and abs(L[2] - A / 2) < 1e-15
+    assert abs(L[3] - A / 10) < 1e-15 and abs(L[4] - A / 10) < 1e-15
+    Gs = oracle.sensor_response(V, 1, [oracle.sensor_params("gaussian", v0, w, A)])["S"][:, 0]
+    assert Gs[0] == A and abs(Gs[1] - A * np.exp(-0.5)) < 1e-15 and abs(Gs[1] - Gs[2]) < 1e-15
+    assert abs(Gs[3] - A * np.exp(-4.5)) < 1e-15
+    lin = oracle.sensor_response(V, 1, [oracle.sensor_params("linear", v0, w, A)])["S"][:, 0]
+    assert np.allclose(lin, A * (V[:, 0] - v0) / w, rtol=0, atol=1e-12)
+    # curvature at the peak: Lorentzian -2A/w^2, Gaussian -A/w^2
+    h = 1e-4
+    assert abs((L[5] + L[6] - 2 * L[0]) / h ** 2 - (-2 * A / w ** 2)) < 1e-2 * A / w ** 2
+    assert abs((Gs[5] + Gs[6] - 2 * Gs[0]) / h ** 2 - (-A / w ** 2)) < 1e-2 * A / w ** 2
+
+
+def test_P14_counter_based_generator():
+    """SplitMix64: the first output of the generator seeded with 0 is 0xE220A8397B1DCDAF (published test vector) -- the inner
+    stage of r(seed=0, stream=0, .).  The composition, the (0,1) mapping and Box-Muller are re-derived here with Python
+    integers / math (exact integer arithmetic modulo 2^64)."""
+    import math
+    MASK, GOLD = (1 << 64) - 1, 0x9E3779B97F4A7C15
+
+    def mix(z):
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & MASK
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & MASK
+        return z ^ (z >> 31)
+
+    assert mix(GOLD) == 0xE220A8397B1DCDAF
+    for seed, stream, idx in ((0, 0, 0), (12345, 7, 99), (2 ** 63 + 5, 200, 2 ** 40 + 3)):
+        r = mix((mix((seed + GOLD * (stream + 1)) & MASK) + GOLD * (idx + 1)) & MASK)
+        assert oracle.rng_u64(seed, stream, idx) == r
+        assert oracle.rng_uniform(seed, stream, idx) == ((r >> 11) + 0.5) * 2.0 ** -53
+    u1, u2 = oracle.rng_uniform(5, 6, 11), oracle.rng_uniform(5, 7, 11)
+    assert abs(oracle.rng_normal(5, 3, 11) - math.sqrt(-2 * math.log(u1)) * math.cos(2 * math.pi * u2)) < 1e-14
+    # different (stream, idx) give different numbers; uniforms fill (0,1) evenly
+    u = np.array([oracle.rng_uniform(1, 0, i) for i in range(20000)])
+    assert 0 < u.min() and u.max() < 1 and abs(u.mean() - 0.5) < 0.01 and abs(u.var() - 1 / 12) < 0.005
+    assert len({oracle.rng_u64(1, s, i) for s in range(8) for i in range(100)}) == 800
+
+
+def test_P14_noise_statistics():
+    """White: zero mean, variance sigma^2, flat spectrum.  1/f (Voss-McCartney, K octaves): variance sigma_p^2, octave j is
+    constant over blocks of 2^j pixels, power spectral density falls with frequency (log-log slope about -1).  Jumps: the
+    baseline is piecewise constant, the number of steps is Binomial(P, rate), step sizes have standard deviation sigma_j."""
+    P = 1 << 16
+    V = np.zeros((P, 1))
+    base = dict(profile="linear", v0=0.0, width=1.0, amplitude=0.0)
+    w = oracle.sensor_response(V, P, [oracle.sensor_params(white_sigma=0.3, seed=11, **base)], False)["S"][:, 0]
+    assert abs(w.mean()) < 4 * 0.3 / np.sqrt(P) and abs(w.var() / 0.09 - 1) < 0.03
+    psd = np.abs(np.fft.rfft(w)) ** 2
+    lo, hi = psd[1:P // 8].mean(), psd[3 * P // 8:].mean()
+    assert abs(lo / hi - 1) < 0.1                                    # flat
+    K = 12
+    pk = oracle.sensor_response(V, P, [oracle.sensor_params(pink_sigma=0.5, pink_octaves=K, seed=12, **base)], False)["S"][:, 0]
+    assert abs(pk.var() / 0.25 - 1) < 0.25 and abs(pk.mean()) < 0.2
+    f = np.fft.rfftfreq(P)[1:]
+    psd = np.abs(np.fft.rfft(pk))[1:] ** 2
+    sel = (f > 2.0 ** -(K - 1)) & (f < 0.25)
+    edges = np.logspace(np.log10(f[sel][0]), np.log10(f[sel][-1]), 12)
+    fc, pc = [], []
+    for a, b in zip(edges[:-1], edges[1:]):
+        m = (f >= a) & (f < b)
+        fc.append(np.sqrt(a * b))
+        pc.append(psd[m].mean())
+    slope = np.polyfit(np.log(fc), np.log(pc), 1)[0]
+    assert -1.4 < slope < -0.6, slope
+    # a single octave j is constant over aligned blocks of 2^j pixels: with K = 1 the noise is white; the difference between
+    # K = 4 and K = 3 signals (rescaled) is the j = 3 source alone
+    s4 = oracle.sensor_response(V, P, [oracle.sensor_params(pink_sigma=2.0, pink_octaves=4, seed=13, **base)], False)["S"][:, 0] * 2.0 / 2.0
+    s3 = oracle.sensor_response(V, P, [oracle.sensor_params(pink_sigma=np.sqrt(3.0), pink_octaves=3, seed=13, **base)], False)["S"][:, 0]
+    src3 = (s4 - s3).reshape(-1, 8)                                  # sigma/sqrt(K) = 1 in both
+    assert np.abs(src3 - src3[:, :1]).max() < 1e-12 and abs(src3[:, 0].var() - 1) < 0.1
+    rate, sj = 0.002, 0.7
+    j = oracle.sensor_response(V, P, [oracle.sensor_params(jump_rate=rate, jump_sigma=sj, seed=14, **base)], False)["S"][:, 0]
+    steps = np.diff(np.concatenate([[0.0], j]))
+    nj = int((steps != 0).sum())
+    assert abs(nj - rate * P) < 5 * np.sqrt(rate * P)
+    assert abs(steps[steps != 0].std() / sj - 1) < 0.25
+    # determinism and independence of the sensors
+    V2 = np.zeros((1000, 2))
+    q = [oracle.sensor_params(white_sigma=1.0, seed=3, **base)] * 2
+    r1, r2 = oracle.sensor_response(V2, 1000, q, False)["S"], oracle.sensor_response(V2, 1000, q, False)["S"]
+    assert np.array_equal(r1, r2) and abs(np.corrcoef(r1[:, 0], r1[:, 1])[0, 1]) < 0.15
+
+
+def test_P14_gradient_is_numpy_gradient_along_the_fast_axis():
+    rng = np.random.default_rng(5)
+    W, H = 37, 11
+    V = rng.uniform(-0.2, 0.2, size=(W * H, 2))
+    q = [oracle.sensor_params("lorentzian", 0.05, 0.03, 1.0, white_sigma=0.01, seed=1),
+         oracle.sensor_params("gaussian", -0.02, 0.05, 2.0, jump_rate=0.01, jump_sigma=0.1, seed=2)]
+    r = oracle.sensor_response(V, W, q)
+    for a in range(2):
+        assert np.allclose(r["G"][:, a].reshape(H, W), np.gradient(r["S"][:, a].reshape(H, W), axis=1), rtol=0, atol=1e-15)
+    assert np.array_equal(oracle.sensor_response(V[:W], 1, q)["G"], np.zeros((W, 2)))
+    with pytest.raises(ValueError):
+        oracle.sensor_response(V, W + 1, q)
+    with pytest.raises(ValueError):
+        oracle.sensor_response(V, W, [oracle.sensor_params(width=0.0)] * 2)
