@@ -155,6 +155,47 @@ QA_API qa_status qa_thermal_closed(const qa_model *model, const double *d_Vg, in
                                    int n_max, double kT, double *d_Nmean, double *d_Emin, qa_stats *d_stats,
                                    void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- charge-sensor response and noise (section IV.A, Fig. 3; reading R14) ------------------ */
+
+/* L149: "we compute the charge sensor's response based on Lorentzian or an approximately Gaussian profile in the weak and
+ * strong coupling regimes ... whilst white, 1/f, and sensor jump noise can be added on top"; L464: the figures show the
+ * derivative of the sensor signal along the swept gate, and a qpc is modelled by "a linear function" instead.  The paper
+ * gives no formula or parameter; reading R14 fixes them and every parameter is the caller's.  With x = (V_s - v0) / width:
+ *   QA_PROFILE_LORENTZIAN  S = amplitude / (1 + x^2)            width = half width at half maximum
+ *   QA_PROFILE_GAUSSIAN    S = amplitude exp(-x^2 / 2)          width = standard deviation
+ *   QA_PROFILE_LINEAR      S = amplitude x
+ * plus, in pixel order p (the raster is the time axis): white noise white_sigma z; 1/f noise pink_sigma / sqrt(K) times
+ * the sum of K = pink_octaves sources, source j redrawn every 2^j pixels (Voss-McCartney); jump noise: at every pixel,
+ * with probability jump_rate, the baseline shifts by jump_sigma z and keeps the shift.  The random numbers are counter
+ * based (SplitMix64 finaliser of seed, stream and index; Box-Muller), so the result depends on `seed` only. */
+typedef enum { QA_PROFILE_LORENTZIAN = 0, QA_PROFILE_GAUSSIAN = 1, QA_PROFILE_LINEAR = 2 } qa_sensor_profile;
+typedef struct {
+    int32_t profile;      /* qa_sensor_profile                                  */
+    int32_t pink_octaves; /* K in [0, 30]                                       */
+    double v0;            /* peak position, in the units of V_s                 */
+    double width;         /* > 0                                                */
+    double amplitude;
+    double white_sigma;   /* >= 0; 0 switches the term off                      */
+    double pink_sigma;    /* >= 0                                               */
+    double jump_rate;     /* probability per pixel, in [0, 1]                   */
+    double jump_sigma;    /* >= 0                                               */
+    uint64_t seed;
+} qa_sensor_params;
+
+/* Device scratch for qa_sensor_response on P pixels and n_sensor sensors (256-byte aligned buffer). */
+QA_API size_t qa_sensor_response_workspace_bytes(int64_t P, int n_sensor);
+
+/*   d_Vsensor  device [P*n_sensor]   sensor potentials (the d_Vsensor output of a ground-state call)
+ *   W          length of the fast axis of the sweep (P must be a multiple of W); only the gradient reads it
+ *   params     HOST, n_sensor entries (1 <= n_sensor <= 16)
+ *   d_signal   device [P*n_sensor]   response + noise
+ *   d_gradient device [P*n_sensor] or NULL: along the fast axis, central differences inside a row, one-sided at its
+ *              ends, in signal units per pixel, of the noisy signal
+ * Asynchronous on cuda_stream; never allocates.  QA_ERR_INVALID_ARG for a parameter outside its range. */
+QA_API qa_status qa_sensor_response(const double *d_Vsensor, int64_t P, int n_sensor, int64_t W, const qa_sensor_params *params,
+                                    double *d_signal, double *d_gradient, void *d_workspace, size_t workspace_bytes,
+                                    void *cuda_stream);
+
 /* ---- dataset batch (BASELINE.json configs[4]) ------------------------------------------------------------------------ */
 
 /* A list of models that share n_dot (<= 8) and n_gate, have no sensor dots and live on the same device.  A batch call

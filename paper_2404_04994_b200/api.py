@@ -24,7 +24,8 @@ EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "q
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
            "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
            "qa_get_kernel_timings", "qa_model_set_walk_variant", "qa_batch_create", "qa_batch_destroy", "qa_batch_size",
-           "qa_ground_state_batch", "qa_thermal_open", "qa_thermal_closed", "qa_last_launch_plan",
+           "qa_ground_state_batch", "qa_thermal_open", "qa_thermal_closed", "qa_sensor_response",
+           "qa_sensor_response_workspace_bytes", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
 
 
@@ -35,6 +36,23 @@ class qa_stats(C.Structure):
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+class qa_sensor_params(C.Structure):
+    """include/qarray_b200.h qa_sensor_params (reading R14)."""
+    _fields_ = [("profile", C.c_int32), ("pink_octaves", C.c_int32), ("v0", C.c_double), ("width", C.c_double),
+                ("amplitude", C.c_double), ("white_sigma", C.c_double), ("pink_sigma", C.c_double),
+                ("jump_rate", C.c_double), ("jump_sigma", C.c_double), ("seed", C.c_uint64)]
+
+
+PROFILE = {"lorentzian": 0, "gaussian": 1, "linear": 2}
+
+
+def sensor_params(profile="lorentzian", v0=0.0, width=1.0, amplitude=1.0, white_sigma=0.0, pink_sigma=0.0, pink_octaves=0,
+                  jump_rate=0.0, jump_sigma=0.0, seed=0) -> qa_sensor_params:
+    return qa_sensor_params(PROFILE[profile] if isinstance(profile, str) else int(profile), int(pink_octaves), float(v0),
+                            float(width), float(amplitude), float(white_sigma), float(pink_sigma), float(jump_rate),
+                            float(jump_sigma), int(seed))
 
 
 class QaError(RuntimeError):
@@ -79,6 +97,9 @@ def lib() -> C.CDLL:
         l.qa_thermal_open.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp, vp, vp, C.c_size_t, vp]
         l.qa_thermal_closed.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp, vp, vp,
                                         C.c_size_t, vp]
+        l.qa_sensor_response_workspace_bytes.argtypes = [C.c_int64, C.c_int]
+        l.qa_sensor_response_workspace_bytes.restype = C.c_size_t
+        l.qa_sensor_response.argtypes = [dp, C.c_int64, C.c_int, C.c_int64, vp, dp, dp, vp, C.c_size_t, vp]
         l.qa_measure_fp64_rate.argtypes = [C.c_double, C.POINTER(C.c_double), vp]
         l.qa_set_kernel_timing.argtypes = [C.c_int]
         l.qa_model_set_walk_variant.argtypes = [vp, C.c_int]
@@ -327,6 +348,27 @@ class Batch:
         if st is not None:
             res["stats"] = st
         return res
+
+
+def sensor_response(Vs: torch.Tensor, W: int, params, want_gradient=True, stream=None) -> dict:
+    """qa_sensor_response on a CUDA tensor Vs[P, n_sensor] (float64; the Vsensor output of a ground-state call): response
+    profile + noise of every sensor (params: one qa_sensor_params per sensor) and the gradient along the fast axis (row
+    length W).  Returns dict(S[P, n_sensor][, G[P, n_sensor]])."""
+    if not (isinstance(Vs, torch.Tensor) and Vs.is_cuda and Vs.dtype == torch.float64):
+        raise TypeError("Vs must be a CUDA float64 tensor (there is no CPU path)")
+    Vs = Vs.contiguous()
+    Vs = Vs.view(Vs.shape[0], -1)
+    P, ns = Vs.shape
+    dev = Vs.device
+    arr = (qa_sensor_params * ns)(*params)
+    S = torch.empty((P, ns), dtype=torch.float64, device=dev)
+    G = torch.empty((P, ns), dtype=torch.float64, device=dev) if want_gradient else None
+    ws = torch.empty(max(256, int(lib().qa_sensor_response_workspace_bytes(P, ns))), dtype=torch.uint8, device=dev)
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.device(dev):
+        _check(lib().qa_sensor_response(_ptr(Vs), P, ns, int(W), C.byref(arr), _ptr(S), _ptr(G), _ptr(ws), ws.numel(),
+                                        C.c_void_p(s.cuda_stream)), "qa_sensor_response")
+    return {"S": S, "G": G} if want_gradient else {"S": S}
 
 
 def stats_dict(t: torch.Tensor) -> dict:

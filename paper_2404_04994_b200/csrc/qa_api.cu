@@ -551,6 +551,39 @@ qa_status qa_thermal_closed(const qa_model *m, const double *d_Vg, int64_t P, in
                    cuda_stream);
 }
 
+size_t qa_sensor_response_workspace_bytes(int64_t P, int n_sensor)
+{
+    if (P < 0 || n_sensor < 1 || n_sensor > QA_MAXN) return 0;
+    return qa_sensor_workspace_bytes_impl(P, n_sensor);
+}
+
+qa_status qa_sensor_response(const double *d_Vsensor, int64_t P, int n_sensor, int64_t W, const qa_sensor_params *params,
+                             double *d_signal, double *d_gradient, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    qa_plan_reset();
+    if (P < 0 || n_sensor < 1 || n_sensor > QA_MAXN || !params || W < 1 || (P % W) != 0) return QA_ERR_INVALID_ARG;
+    if (P > 0 && (!d_Vsensor || !d_signal)) return QA_ERR_INVALID_ARG;
+    for (int a = 0; a < n_sensor; ++a) {
+        const qa_sensor_params &q = params[a];
+        if (q.profile < 0 || q.profile > 2 || !(q.width > 0.0) || !std::isfinite(q.width) || q.pink_octaves < 0 ||
+            q.pink_octaves > 30 || !(q.white_sigma >= 0.0) || !(q.pink_sigma >= 0.0) || !(q.jump_sigma >= 0.0) ||
+            !(q.jump_rate >= 0.0 && q.jump_rate <= 1.0) || !std::isfinite(q.v0) || !std::isfinite(q.amplitude))
+            return QA_ERR_INVALID_ARG;
+    }
+    if (P == 0) return QA_OK;
+    if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
+    if (!d_workspace || workspace_bytes < qa_sensor_workspace_bytes_impl(P, n_sensor) ||
+        (reinterpret_cast<uintptr_t>(d_workspace) & 255u))
+        return QA_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    g_n_marks = 0;
+    timing_mark(stream);
+    QA_CUDA(qa_launch_sensor_response(params, n_sensor, d_Vsensor, P, W, d_signal, d_gradient,
+                                      static_cast<double *>(d_workspace), stream));
+    timing_mark(stream);
+    return QA_OK;
+}
+
 qa_status qa_batch_create(const qa_model *const *models, int n_models, qa_batch **out)
 {
     if (out) *out = nullptr;

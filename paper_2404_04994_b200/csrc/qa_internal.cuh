@@ -97,6 +97,9 @@ cudaError_t qa_launch_thermal(const QaDevModel *d_model, int n, QaWorkspace ws, 
                               double expect_cand, double *d_Nmean, double *d_Emin, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
                                double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream);
+cudaError_t qa_launch_sensor_response(const qa_sensor_params *params, int ns, const double *d_Vs, int64_t P, int64_t W,
+                                      double *d_S, double *d_G, double *d_partial, cudaStream_t stream);
+size_t qa_sensor_workspace_bytes_impl(int64_t P, int ns);
 cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int iters, cudaStream_t stream);
 
 // ---- small device helpers ------------------------------------------------------------------------------------------

@@ -539,3 +539,59 @@ def test_full_size_config5_every_member_every_pixel(api):
     256 members x 3 algorithms, every pixel against the oracle (3 x 4.19 M pixel searches)."""
     rep = full_size_report(api, oracle, wl, torch, strict=True, configs=(5,))["config5"]
     assert rep["pixels"] == 3 * 256 * 128 * 128 and rep["unexcused"] == 0 and rep["qp_pixels"] > 0
+
+
+# ---- charge-sensor response, noise and gradient (SURVEY 8(f) NEXT-2; reading R14) ------------------------------------
+@pytest.mark.parametrize("W,H", [(200, 200), (37, 29), (1, 5), (4099, 3)])
+def test_sensor_response_config3_profiles_noise_gradient(api, W, H):
+    """qa_sensor_response on the sensor potential of config 3 (computed by the CUDA path) against qo_sensor_response on the
+    same potentials: every profile, each noise term alone and all together, gradient included.  Tolerance: 1e-9 of the
+    signal scale (the draws are the same counter-based numbers; log / cos / the order of the jump prefix sum differ in the
+    last bits).  Sizes span several 1024-pixel chunks, ragged tails and rows longer than a chunk."""
+    w = wl.config3(W, H)
+    m = api.Model(w.C_dd, w.C_gd, sensor_dots=w.sensor_dots)
+    r = m.ground_state(torch.from_numpy(w.Vg).cuda())
+    Vs = r["Vsensor"]
+    vs = Vs.cpu().numpy()
+    v0, wd = float(np.median(vs)), float(max(1e-3, 0.3 * (vs.max() - vs.min() + 1e-3)))
+    cases = [dict(profile="lorentzian", v0=v0, width=wd, amplitude=1.5),
+             dict(profile="gaussian", v0=v0, width=wd, amplitude=0.7),
+             dict(profile="linear", v0=v0, width=wd, amplitude=-2.0),
+             dict(profile="lorentzian", v0=v0, width=wd, amplitude=1.0, white_sigma=0.05, seed=5),
+             dict(profile="lorentzian", v0=v0, width=wd, amplitude=1.0, pink_sigma=0.08, pink_octaves=14, seed=6),
+             dict(profile="gaussian", v0=v0, width=wd, amplitude=1.0, jump_rate=0.004, jump_sigma=0.2, seed=7),
+             dict(profile="lorentzian", v0=v0, width=wd, amplitude=1.0, white_sigma=0.02, pink_sigma=0.05, pink_octaves=30,
+                  jump_rate=0.01, jump_sigma=0.1, seed=2 ** 63 + 11)]
+    for kw in cases:
+        g = api.sensor_response(Vs, W, [api.sensor_params(**kw)])
+        torch.cuda.synchronize()
+        o = oracle.sensor_response(vs, W, [oracle.sensor_params(**kw)])
+        scale = abs(kw["amplitude"]) + kw.get("white_sigma", 0) + kw.get("pink_sigma", 0) + np.abs(o["S"]).max()
+        assert np.abs(g["S"].cpu().numpy() - o["S"]).max() <= 1e-9 * scale, kw
+        assert np.abs(g["G"].cpu().numpy() - o["G"]).max() <= 1e-9 * scale, kw
+    if W == 200:
+        assert api.last_launch_plan()[0] == ["qa_sensor_jump_partials_kernel", "qa_sensor_jump_scan_kernel",
+                                             "qa_sensor_signal_kernel", "qa_sensor_gradient_kernel"]
+
+
+def test_sensor_response_two_sensors_long_trace_and_errors(api):
+    """Two sensors with different parameters (independent streams), a trace of 3 * 2^18 pixels (768 chunks: the scan of the
+    chunk sums runs three rounds), no gradient requested; argument errors."""
+    P, W = 3 << 18, 1 << 10
+    rng = np.random.default_rng(3)
+    vs = np.ascontiguousarray(rng.uniform(-0.1, 0.1, size=(P, 2)))
+    Vs = torch.from_numpy(vs).cuda()
+    kws = [dict(profile="lorentzian", v0=0.01, width=0.03, amplitude=1.0, white_sigma=0.01, pink_sigma=0.02, pink_octaves=18,
+                jump_rate=0.0005, jump_sigma=0.3, seed=21),
+           dict(profile="gaussian", v0=-0.02, width=0.05, amplitude=2.0, jump_rate=0.002, jump_sigma=0.1, seed=21)]
+    g = api.sensor_response(Vs, W, [api.sensor_params(**k) for k in kws], want_gradient=False)
+    torch.cuda.synchronize()
+    o = oracle.sensor_response(vs, W, [oracle.sensor_params(**k) for k in kws], want_gradient=False)
+    scale = 2.0 + np.abs(o["S"]).max()
+    assert np.abs(g["S"].cpu().numpy() - o["S"]).max() <= 1e-9 * scale
+    assert "G" not in g
+    for bad in (dict(width=0.0), dict(pink_octaves=31), dict(jump_rate=1.5), dict(white_sigma=-1.0), dict(profile=3)):
+        with pytest.raises(api.QaError):
+            api.sensor_response(Vs, W, [api.sensor_params(**bad)] * 2)
+    with pytest.raises(api.QaError):
+        api.sensor_response(Vs, W + 1, [api.sensor_params()] * 2)
