@@ -336,6 +336,17 @@ qa_status thermal(const qa_model *m, const double *d_Vg, int64_t P, int closed, 
     const double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n)
                           : alg == QA_ALG_DEFAULT   ? std::pow(2.0, (double)n)
                                                     : std::pow(1.0 + t, (double)n);
+    // open default set of a larger Maxwell array: sum-product over the min-plus split, while the factorised weights stay
+    // far from underflow (beta * sum_{i<j} M_ij <= 600, qa_kernels_thermal_sp.cu); otherwise the two-pass kernels
+    double gsum = 0.0;
+    for (int i = 0; i < n; ++i)
+        for (int j = i + 1; j < n; ++j) gsum += std::fabs(m->host.M[i * QA_MAXN + j]);
+    if (!closed && alg == QA_ALG_DEFAULT && n > QA_WALK_NL && m->is_z && gsum / kT <= 600.0 &&
+        m->walk_variant.load(std::memory_order_relaxed) != 0) {
+        QA_CUDA(qa_launch_thermal_sp(m->dev, n, m->host.QL, ws, kT, d_Nmean, d_Emin, m->sm_count, stream));
+        timing_mark(stream);
+        return QA_OK;
+    }
     QA_CUDA(qa_launch_thermal(m->dev, n, ws, a, kT, expect, d_Nmean, d_Emin, d_stats, stream));
     timing_mark(stream);
     return QA_OK;

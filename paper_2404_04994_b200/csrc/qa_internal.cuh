@@ -95,6 +95,8 @@ cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models
                                  qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_thermal(const QaDevModel *d_model, int n, QaWorkspace ws, QaCallArgs args, double kT,
                               double expect_cand, double *d_Nmean, double *d_Emin, qa_stats *d_stats, cudaStream_t stream);
+cudaError_t qa_launch_thermal_sp(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, double kT,
+                                 double *d_Nmean, double *d_Emin, int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
                                double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_sensor_response(const qa_sensor_params *params, int ns, const double *d_Vs, int64_t P, int64_t W,

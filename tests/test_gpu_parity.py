@@ -338,6 +338,42 @@ def test_thermal_all_sizes(api, n, P):
         check_thermal(api, w, 0.08, algorithm="default")
 
 
+@pytest.mark.parametrize("n,P", [(9, 515), (10, 300), (12, 131), (13, 77), (14, 40), (15, 21), (16, 33)])
+def test_thermal_sum_product_kernel(api, n, P):
+    """Open default set of 9..16 dots: the sum-product kernel (qa_thermal_sp_kernel, factorised Boltzmann weights over the
+    min-plus split) against the oracle at a warm and a cool temperature, and against the two-pass Gray kernel (variant 0 of
+    the model) on the same pixels; at a temperature so low that the factorised weights could underflow the launcher must
+    fall back to the Gray kernel by itself."""
+    w = wl.random_open(n, n, P, seed=650 + n, lo=-0.4, hi=2.6)
+    M = np.linalg.inv(w.C_dd)
+    gsum = np.abs(np.triu(M, 1)).sum()
+    EC = 0.5 * np.diag(M).min()
+    for kT_over_EC in (0.3, max(0.05, 1.05 * gsum / 600.0 / EC)):
+        Nm, o = check_thermal(api, w, kT_over_EC, algorithm="default")
+        assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_sp_kernel"]
+        m0 = api.Model(w.C_dd, w.C_gd, walk_variant=0)
+        r0 = m0.thermal(torch.from_numpy(w.Vg).cuda(), kT_over_EC * EC)
+        assert api.last_launch_plan()[0][1].startswith("qa_thermal_gray_kernel")
+        assert np.abs(r0["Nmean"].cpu().numpy() - Nm).max() <= 1e-9 * max(1.0, 0.02 / kT_over_EC) * max(1.0, np.abs(Nm).max())
+    check_thermal(api, w, 0.9 * gsum / 600.0 / EC, algorithm="default")
+    assert api.last_launch_plan()[0][1].startswith("qa_thermal_gray_kernel")
+
+
+def test_thermal_sum_product_full_size_sample(api):
+    """bench.py's thermal workload (config 4, 100x100, kT = 0.05 E_C) in its launch configuration: 300 seeded pixels of the
+    full diagram against the oracle."""
+    w = wl.config4(100, 100)
+    m = api.Model(w.C_dd, w.C_gd)
+    om = oracle.Model(w.C_dd, w.C_gd)
+    kT = 0.05 * om.EC
+    r = m.thermal(torch.from_numpy(w.Vg).cuda(), kT)
+    assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_sp_kernel"]
+    sel = np.sort(np.random.default_rng(1).choice(w.P, size=300, replace=False))
+    o = om.thermal(w.Vg[sel], kT)
+    assert np.abs(r["Nmean"].cpu().numpy()[sel] - o["Nmean"]).max() <= 1e-9 * max(1.0, np.abs(o["Nmean"]).max())
+    assert np.abs(r["Emin"].cpu().numpy()[sel] - o["Emin"]).max() <= 1e-9 * max(om.EC, np.abs(o["Emin"]).max())
+
+
 def test_thermal_cold_limit_is_the_ground_state_and_errors(api):
     w = wl.config5_array(1, 40, 40)
     m = api.Model(w.C_dd, w.C_gd)
