@@ -275,7 +275,7 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
             return QA_OK;
         }
     }
-    QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream));
+    QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream, variant != 0));
     timing_mark(stream);
     // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd
     if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && variant != 0 && m->is_z) {
@@ -331,7 +331,8 @@ qa_status thermal(const qa_model *m, const double *d_Vg, int64_t P, int closed, 
     QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1};
     g_n_marks = 0;
     timing_mark(stream);
-    QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, nullptr, d_stats, stream));
+    QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, nullptr, d_stats, stream,
+                               m->walk_variant.load(std::memory_order_relaxed) != 0));
     timing_mark(stream);
     const double expect = alg == QA_ALG_BRUTE_FORCE ? std::pow((double)n_max + 1.0, (double)n)
                           : alg == QA_ALG_DEFAULT   ? std::pow(2.0, (double)n)

@@ -78,7 +78,7 @@ void qa_timing_mark(cudaStream_t stream);  // measurement aid: event between two
 
 // launchers (each enqueues exactly one kernel on `stream` and logs it)
 cudaError_t qa_launch_prologue(const QaDevModel *d_model, int n, int g, const double *d_Vg, QaWorkspace ws,
-                               QaCallArgs args, double *d_xcont, qa_stats *d_stats, cudaStream_t stream);
+                               QaCallArgs args, double *d_xcont, qa_stats *d_stats, cudaStream_t stream, bool lanes = false);
 cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws, QaCallArgs args, double expect_cand,
                                 qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, qa_stats *d_stats,

@@ -87,6 +87,199 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// Prologue of OPEN arrays with 9..16 dots, sixteen lanes per pixel (lane i <-> dot i).  The thread-per-pixel kernel above
+// puts 10^4 pixels on 79 CTAs -- two warps per SM, each thread a chain of ~600 dependent FP64 instructions.  Here a pixel's
+// N_c,i (the same fma chain over k as everywhere: reading R1), the candidate range of dot i and the row i of M d0 belong
+// to lane i, the other dots' values travel by shuffles, and the outputs go through shared memory so that the stores to
+// the [i][P] workspace stay coalesced.  The QP (L106, reading R3) runs the clamp-only active set with every lane of the
+// pixel solving the same 1x1 / 2x2 / 3x3 system in registers (qa_qp_small_open's formulas); larger active sets and
+// non-Maxwell models go to the serial solver on the pixel's first lane.
+// The serial QP of one pixel on its own frame: cx holds N_c on entry and the constrained minimum on return.
+template <int N>
+__device__ __noinline__ void pl_slow_qp(const double *__restrict__ sC, double *cx, bool general, int *st)
+{
+    double c[N], xs[N];
+    for (int j = 0; j < N; ++j) c[j] = xs[j] = cx[j];
+    bool failed = false;
+    st[0] = qa_qp_clamp<N>(sC, c, false, 0.0, general, xs, failed);
+    st[1] = failed ? 1 : 0;
+    for (int j = 0; j < N; ++j) cx[j] = xs[j];
+}
+
+template <int N>
+__global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel *__restrict__ mdl,
+                                                                const double *__restrict__ Vg, QaWorkspace ws, QaCallArgs args,
+                                                                double *__restrict__ xcont, qa_stats *stats)
+{
+    constexpr int LPP = 16, PPB = 256 / LPP;
+    static_assert(N > 8 && N <= LPP, "sixteen lanes per pixel");
+    __shared__ double sCgT[QA_MAXG * N], sC[N * N], sMT[N * N], sV[PPB][QA_MAXG];
+    __shared__ double sH[N][PPB], sNc[N][PPB], sX[PPB][N];
+    __shared__ int32_t sBase[N][PPB], sCnt[N][PPB];
+    const int g = mdl->g;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < N * N; e += 256) {
+        sMT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
+        sC[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
+    }
+    for (int e = tid; e < N * g; e += 256) sCgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
+    const int64_t P = ws.P;
+    const int64_t p0 = (int64_t)blockIdx.x * PPB;
+    for (int e = tid; e < PPB * g; e += 256) {
+        const int64_t pe = p0 + e / g;
+        sV[e / g][e % g] = pe < P ? __ldg(Vg + p0 * g + e) : 0.0;
+    }
+    __syncthreads();
+    qa_pdl_launch_dependents();
+    if (blockIdx.x == 0 && tid == 0) *ws.counter = 0ull;  // work counter of the pruned min-plus walk
+
+    const int i = tid & (LPP - 1);          // dot
+    const int s = tid >> 4;                 // pixel slot
+    const unsigned lane = tid & 31u;
+    const int gb = (int)(lane & 16u);       // first lane of the pixel's group inside the warp
+    const int64_t p = p0 + s;
+    const bool live = p < P;
+    const bool dot = i < N;
+    const int ii = dot ? i : 0;
+
+    // S1 (R1): N_c,i = fma(C_gd[i,k], V[k], acc), k ascending
+    double nc = 0.0;
+    for (int k = 0; k < g; ++k) nc = fma(sCgT[k * N + ii], sV[s][k], nc);
+    // S2 (open): x = N_c.  S3: clamp-only active set
+    double x = nc;
+    int rounds = 0;
+    bool failed = false, slow = false;
+    const unsigned neg0 = (__ballot_sync(0xffffffffu, dot && x < 0.0) >> gb) & 0xffffu;
+    if (__any_sync(0xffffffffu, neg0 != 0u)) {
+        double scale = fabs(nc);
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) scale = fmax(scale, __shfl_xor_sync(0xffffffffu, scale, o));
+        scale = fmax(scale, 1.0);
+        unsigned A = 0;
+        bool done = neg0 == 0u;
+        slow = !done && args.general_qp != 0;
+        for (;;) {
+            const unsigned negm = (__ballot_sync(0xffffffffu, dot && x < 0.0) >> gb) & 0xffffu & ~A;
+            if (!done && !slow) {
+                if (!negm) {
+                    done = true;
+                } else {
+                    A |= negm;
+                    ++rounds;
+                    if (__popc(A) == N) {
+                        x = 0.0;
+                        done = true;
+                    } else if (__popc(A) > 3) {
+                        slow = true;
+                    }
+                }
+            }
+            const bool work = !done && !slow;
+            if (!__any_sync(0xffffffffu, work)) break;
+            // closed form for |A| <= 3 (every lane of the pixel computes the same y): qa_qp_small_open's arithmetic
+            const unsigned Aw = work ? A : 1u;
+            const int ia = __ffs(Aw) - 1;
+            const unsigned A2 = Aw & (Aw - 1);
+            const int ib = A2 ? __ffs(A2) - 1 : ia;
+            const unsigned A3 = A2 & (A2 - 1);
+            const int ic = A3 ? __ffs(A3) - 1 : ib;
+            const double ca = __shfl_sync(0xffffffffu, nc, gb + ia), cb = __shfl_sync(0xffffffffu, nc, gb + ib),
+                         cc = __shfl_sync(0xffffffffu, nc, gb + ic);
+            if (work) {
+                double ya, yb = 0.0, yc = 0.0;
+                if (A3) {
+                    const double a = sC[ia * N + ia], b = sC[ia * N + ib], cq = sC[ia * N + ic];
+                    const double d = sC[ib * N + ib], e = sC[ib * N + ic], f = sC[ic * N + ic];
+                    const double k00 = d * f - e * e, k01 = cq * e - b * f, k02 = b * e - cq * d;
+                    const double k11 = a * f - cq * cq, k12 = b * cq - a * e, k22 = a * d - b * b;
+                    const double det = a * k00 + b * k01 + cq * k02;
+                    ya = -(k00 * ca + k01 * cb + k02 * cc) / det;
+                    yb = -(k01 * ca + k11 * cb + k12 * cc) / det;
+                    yc = -(k02 * ca + k12 * cb + k22 * cc) / det;
+                } else if (A2) {
+                    const double Caa = sC[ia * N + ia], Cab = sC[ia * N + ib], Cbb = sC[ib * N + ib];
+                    const double det = Caa * Cbb - Cab * Cab;
+                    ya = (cb * Cab - ca * Cbb) / det;
+                    yb = (ca * Cab - cb * Caa) / det;
+                } else {
+                    ya = -ca / sC[ia * N + ia];
+                }
+                double sx = nc + sC[ii * N + ia] * ya;
+                if (A2) sx += sC[ii * N + ib] * yb;
+                if (A3) sx += sC[ii * N + ic] * yc;
+                x = ((A >> i) & 1u) ? 0.0 : sx;  // clamped components are exactly 0 (R3)
+                if (ya < -1e-9 * scale || yb < -1e-9 * scale || yc < -1e-9 * scale) failed = true;  // KKT
+            }
+        }
+        // more than three clamped dots, or a c_dd with a positive off-diagonal: the serial solver on the pixel's first lane
+        if (__any_sync(0xffffffffu, slow)) {
+            if (slow && dot) sX[s][i] = nc;
+            __syncwarp();
+            if (slow && i == 0) {
+                int st2[2];
+                pl_slow_qp<N>(sC, sX[s], args.general_qp != 0, st2);
+                rounds = st2[0];
+                failed = st2[1] != 0;
+            }
+            __syncwarp();
+            if (slow && dot) x = sX[s][i];
+        }
+    }
+    // S4: candidate range of dot i
+    int32_t base = 0, cnt = 1;
+    if (dot) {
+        if (args.alg == QA_ALG_BRUTE_FORCE) {
+            base = 0;
+            cnt = args.n_max + 1;
+        } else {
+            qa_floor_ceil(x, args.t, args.alg == QA_ALG_THRESHOLDED, base, cnt);
+        }
+    }
+    const double d0 = dot ? (double)base - nc : 0.0;
+    // base-point gradient: row i of M d0 (j ascending), h_i = grad_i + 1/2 M_ii, E(base) = 1/2 sum_i d0_i grad_i
+    double gi = 0.0;
+#pragma unroll
+    for (int j = 0; j < N; ++j) gi = fma(sMT[j * N + ii], __shfl_sync(0xffffffffu, d0, gb + j), gi);
+    double e0 = dot ? d0 * gi : 0.0;
+    uint64_t total = (uint64_t)cnt;
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {
+        e0 += __shfl_xor_sync(0xffffffffu, e0, o);
+        total *= __shfl_xor_sync(0xffffffffu, total, o);
+    }
+    if (dot) {
+        sH[i][s] = gi + 0.5 * sMT[i * N + i];
+        sNc[i][s] = nc;
+        sBase[i][s] = base;
+        sCnt[i][s] = cnt;
+        if (live && xcont) xcont[p * N + i] = x;
+    }
+    if (live && i == 0) {
+        ws.total[p] = total;
+        ws.e0[p] = 0.5 * e0;
+    }
+    __syncthreads();
+    {   // coalesced stores: thread (row r, column c) of the [N][PPB] tiles
+        const int r = tid >> 4, c = tid & 15;
+        if (r < N && p0 + c < P) {
+            ws.h[(int64_t)r * P + p0 + c] = sH[r][c];
+            ws.nc[(int64_t)r * P + p0 + c] = sNc[r][c];
+            ws.base[(int64_t)r * P + p0 + c] = sBase[r][c];
+            ws.cnt[(int64_t)r * P + p0 + c] = sCnt[r][c];
+        }
+    }
+    if (stats) {
+        const bool one = live && i == 0;
+        qa_warp_count(&stats->n_pixels, one ? 1 : 0);
+        qa_warp_count(&stats->n_qp_pixels, (one && neg0 != 0u) ? 1 : 0);
+        qa_warp_count(&stats->n_qp_rounds, one ? rounds : 0);
+        qa_warp_count(&stats->n_qp_failed, (one && failed) ? 1 : 0);
+        qa_warp_count(&stats->n_candidates_enumerated, one ? (int64_t)total : 0);
+        qa_warp_count(&stats->n_candidates_scored, one ? (int64_t)total : 0);  // open: all are scored
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // Generic enumeration (every algorithm and regime): the candidate set of a pixel is the box prod_i [base_i, base_i +
 // cnt_i), enumerated in lexicographic order (dot 0 most significant) as a mixed-radix odometer.  G threads share a pixel;
 // each takes a contiguous chunk of the index range, builds its first candidate from the definition (d = N - N_c,
@@ -274,6 +467,15 @@ cudaError_t launch_prologue_n(const QaDevModel *d_model, const double *d_Vg, QaW
 }
 
 template <int N>
+cudaError_t launch_prologue_lanes_n(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, QaCallArgs args,
+                                    double *d_xcont, qa_stats *d_stats, cudaStream_t stream)
+{
+    const unsigned blocks = (unsigned)((ws.P + 15) / 16);
+    qa_prologue_lanes_kernel<N><<<blocks, 256, 0, stream>>>(d_model, d_Vg, ws, args, d_xcont, d_stats);
+    return cudaGetLastError();
+}
+
+template <int N>
 cudaError_t launch_enumerate_n(const QaDevModel *d_model, QaWorkspace ws, QaCallArgs args, double expect_cand,
                                qa_stats *d_stats, cudaStream_t stream)
 {
@@ -325,9 +527,25 @@ cudaError_t launch_enumerate_n(const QaDevModel *d_model, QaWorkspace ws, QaCall
     }
 
 cudaError_t qa_launch_prologue(const QaDevModel *d_model, int n, int g, const double *d_Vg, QaWorkspace ws,
-                               QaCallArgs args, double *d_xcont, qa_stats *d_stats, cudaStream_t stream)
+                               QaCallArgs args, double *d_xcont, qa_stats *d_stats, cudaStream_t stream, bool lanes)
 {
     (void)g;
+    if (lanes && !args.closed && n > 8) {  // open arrays of 9..16 dots: sixteen lanes per pixel
+        qa_plan_add("qa_prologue_lanes_kernel");
+#define CALL(NN) launch_prologue_lanes_n<NN>(d_model, d_Vg, ws, args, d_xcont, d_stats, stream)
+        switch (n) {
+            case 9: return CALL(9);
+            case 10: return CALL(10);
+            case 11: return CALL(11);
+            case 12: return CALL(12);
+            case 13: return CALL(13);
+            case 14: return CALL(14);
+            case 15: return CALL(15);
+            case 16: return CALL(16);
+            default: return cudaErrorInvalidValue;
+        }
+#undef CALL
+    }
     qa_plan_add("qa_prologue_kernel");
 #define CALL(NN) launch_prologue_n<NN>(d_model, d_Vg, ws, args, d_xcont, d_stats, stream)
     QA_DISPATCH_N(n, CALL)

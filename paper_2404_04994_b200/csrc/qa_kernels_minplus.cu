@@ -43,7 +43,7 @@
 namespace {
 
 constexpr int MP_THREADS = 256;
-constexpr int MF_THREADS = 128;
+constexpr int MF_THREADS = 256;
 
 template <int NL>
 struct alignas(16) MpTable {
@@ -462,10 +462,13 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_pruned_kernel(con
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
-// pass 2 + S7: one warp per pixel.  The code runs once per warp (10^4 warps at config 4), so what it pays for is the
-// instruction count and the MIO queue (shuffles, loads), not arithmetic: every lane loads the pixel's inputs itself
-// (warp-uniform addresses, one L1 request each) instead of trading them by shuffle, the survivor's constants come from
-// the model tables, and each lane scores a block of CPL consecutive candidates with a static add tree.
+// pass 2 + S7: one warp per pixel, PERSISTENT warps.  A pixel costs a warp a chain of dependent steps (records -> minimum ->
+// survivor -> its constants -> 2^NL candidates -> lexicographic minimum -> N*, E(N*)), so what the kernel pays for is
+// latency, not arithmetic.  Hence: every warp walks pixels gw, gw + #warps, ... and requests the inputs of its NEXT pixel
+// (one value per lane: h_lane or E(base); the warp records; base and N_c of the lane's dot) before it works on the current
+// one, whose inputs sit in shared memory; the survivor's constants (VT[t], QHT[t]) are read from the model tables the walk
+// kernel has just left in L2, lane i keeps row i of M in registers for S7, and each lane scores a block of CPL consecutive
+// candidates with a static add tree.
 template <int NH, int NU, int NW>
 __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaDevModel *__restrict__ mdl,
                                                                        QaWorkspace ws, int32_t *__restrict__ outN,
@@ -476,138 +479,168 @@ __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaD
     constexpr int WPP = (1 << NH) / 32;
     constexpr int LB = NL - 5;          // log2 of the candidates per lane
     constexpr int CPL = 1 << LB;        // candidates per lane: w = (wb << LB) + c, one u per lane
+    constexpr int WARPS = MF_THREADS / 32;
     static_assert(LB >= 1 && LB <= NW, "a lane's block of candidates lies inside one u");
-    __shared__ double sd[MF_THREADS / 32][QA_MAXN];
-    __shared__ double sM[N][N];
+    __shared__ double sIn[WARPS][N + 1];   // h[0..N-1], E(base) of the warp's current pixel
+    __shared__ double sd[WARPS][QA_MAXN];
     const unsigned lane = threadIdx.x & 31u;
     const int wid = threadIdx.x >> 5;
     const int64_t P = ws.P;
-    const int64_t p = (int64_t)blockIdx.x * (MF_THREADS / 32) + wid;
-    const bool live = p < P;
-    const int64_t pp = live ? p : P - 1;
+    const int64_t gw = (int64_t)wid * gridDim.x + blockIdx.x;   // consecutive warps sit in different CTAs (ragged tail)
+    const int64_t tw = (int64_t)gridDim.x * WARPS;
 
-    // Everything that does not depend on the survivor is requested up front, in one round trip: the warp records, the
-    // pixel's inputs (every lane all of them: warp-uniform addresses, one L1 request each), the lane's table entries,
-    // base / N_c of the lane's dot, and M (staged in shared memory for S7).
+    // model constants: the lane's table entries, row `lane` of M, and the survivor tables in shared memory
     const double EC = mdl->EC;
     double2 ql[CPL / 2];
 #pragma unroll
     for (int c = 0; c < CPL / 2; ++c) ql[c] = reinterpret_cast<const double2 *>(mdl->QL + lane * CPL)[c];
-    for (int e = threadIdx.x; e < N * N; e += MF_THREADS) sM[e / N][e % N] = mdl->M[(e / N) * QA_MAXN + (e % N)];
+    double Mrow[N];
+    {
+        const int li = lane < (unsigned)N ? (int)lane : 0;
+#pragma unroll
+        for (int j = 0; j < N; ++j) Mrow[j] = mdl->M[li * QA_MAXN + j];
+    }
     qa_pdl_wait();  // model constants above; everything below was written by the prologue / walk kernels
-    uint2 r = make_uint2(0xffffffffu, 0u);
-    if (lane < WPP) r = ws.rec[pp * WPP + lane];
-    double h[N];
-#pragma unroll
-    for (int i = 0; i < N; ++i) h[i] = __ldg(ws.h + (int64_t)i * P + pp);
-    const double e0 = __ldg(ws.e0 + pp);
-    int32_t base_i = 0;
-    double nc_i = 0.0;
-    if (lane < N) {
-        base_i = ws.base[(int64_t)lane * P + pp];
-        nc_i = ws.nc[(int64_t)lane * P + pp];
-    }
-    __syncthreads();
-    if (!live) return;
-    const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
-    const unsigned wmask = __ballot_sync(0xffffffffu, lane < WPP && r.x <= H + 2u);  // warps that may hold the argmin
 
-    // thread-independent offsets, as pass 1 formed them (j ascending)
-    double offw = EC, offu = 0.0;
-#pragma unroll
-    for (int j = 0; j < NL; ++j) {
-        if (j < NW)
-            offw += fabs(h[N - 1 - j]);
-        else
-            offu += fabs(h[N - 1 - j]);
-    }
     const unsigned u = lane >> (NW - LB);                         // this lane's u
     const unsigned wb = lane & ((1u << (NW - LB)) - 1u);          // ... and the bits of w above its block
 
-    double bestE = INFINITY;
-    unsigned bestI = 0xffffffffu;
-    for (int q = 0; q < WPP; ++q) {
-        unsigned surv = __shfl_sync(0xffffffffu, r.y, q);
-        if (!((wmask >> q) & 1u)) continue;
-        while (surv) {
-            const unsigned ts = (unsigned)q * 32u + (unsigned)(__ffs(surv) - 1);
-            surv &= surv - 1;
-            // the survivor's inputs as pass 1 built them (same operands, same order)
-            double hp[NL];
+    // inputs of a pixel, one value per lane
+    double in_v = 0.0, in_nc = 0.0;
+    int32_t in_base = 0;
+    uint2 in_r = make_uint2(0xffffffffu, 0u);
+    auto request = [&](int64_t p) {
+        if (p >= P) return;
+        if (lane <= (unsigned)N) in_v = lane < (unsigned)N ? __ldg(ws.h + (int64_t)lane * P + p) : __ldg(ws.e0 + p);
+        if (lane < (unsigned)N) {
+            in_base = ws.base[(int64_t)lane * P + p];
+            in_nc = ws.nc[(int64_t)lane * P + p];
+        }
+        in_r = lane < (unsigned)WPP ? ws.rec[p * WPP + lane] : make_uint2(0xffffffffu, 0u);
+    };
+    request(gw);
+    for (int64_t p = gw; p < P; p += tw) {
+        const uint2 r = in_r;
+        const int32_t base_i = in_base;
+        const double nc_i = in_nc;
+        if (lane <= (unsigned)N) sIn[wid][lane] = in_v;
+        __syncwarp();
+        request(p + tw);
+        const double *__restrict__ h = sIn[wid];
+        const double e0 = h[N];
+        const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
+        const unsigned wmask = __ballot_sync(0xffffffffu, lane < (unsigned)WPP && r.x <= H + 2u);  // warps that may hold the argmin
+
+        // thread-independent offsets, as pass 1 formed them (j ascending)
+        double offw = EC, offu = 0.0;
 #pragma unroll
-            for (int j = 0; j < NL; ++j) hp[j] = h[N - 1 - j] + mdl->VT[ts * NL + j];
-            double be = e0 + mdl->QHT[ts];
+        for (int j = 0; j < NL; ++j) {
+            if (j < NW)
+                offw += fabs(h[N - 1 - j]);
+            else
+                offu += fabs(h[N - 1 - j]);
+        }
+
+        double bestE = INFINITY;
+        unsigned bestI = 0xffffffffu;
+        for (int q = 0; q < WPP; ++q) {
+            unsigned surv = __shfl_sync(0xffffffffu, r.y, q);
+            if (!((wmask >> q) & 1u)) continue;
+            while (surv) {
+                const unsigned ts = (unsigned)q * 32u + (unsigned)(__ffs(surv) - 1);
+                surv &= surv - 1;
+                // the survivor's inputs as pass 1 built them (same operands, same order)
+                double hp[NL];
 #pragma unroll
-            for (int jh = 0; jh < NH; ++jh)
-                if ((ts >> jh) & 1u) be += h[N - 1 - NL - jh];
-            // A[u] = ah[u >> 2] + lo[u & 3]
-            double a = be + offu;
+                for (int j = 0; j < NL; ++j) hp[j] = h[N - 1 - j] + __ldg(mdl->VT + ts * NL + j);
+                double be = e0 + __ldg(mdl->QHT + ts);
 #pragma unroll
-            for (int j = NU - 1; j >= 2; --j)
-                if ((u >> j) & 1u) a += hp[NW + j];
-            if ((u & 3u) == 1u) a += hp[NW];
-            if ((u & 3u) == 2u) a += hp[NW + 1];
-            if ((u & 3u) == 3u) a += hp[NW + 1] + hp[NW];
-            // B[w] of the lane's block: bits of w from the highest down
-            double b[CPL];
-            b[0] = offw;
+                for (int jh = 0; jh < NH; ++jh)
+                    if ((ts >> jh) & 1u) be += h[N - 1 - NL - jh];
+                // A[u] = ah[u >> 2] + lo[u & 3]
+                double a = be + offu;
 #pragma unroll
-            for (int j = NW - 1; j >= LB; --j)
-                if ((wb >> (j - LB)) & 1u) b[0] += hp[j];
+                for (int j = NU - 1; j >= 2; --j)
+                    if ((u >> j) & 1u) a += hp[NW + j];
+                if ((u & 3u) == 1u) a += hp[NW];
+                if ((u & 3u) == 2u) a += hp[NW + 1];
+                if ((u & 3u) == 3u) a += hp[NW + 1] + hp[NW];
+                // B[w] of the lane's block: bits of w from the highest down
+                double b[CPL];
+                b[0] = offw;
 #pragma unroll
-            for (int c = 1; c < CPL; ++c) b[c] = b[c & (c - 1)] + hp[mp_ctz(c)];
-            double e1 = INFINITY;
-            unsigned i1 = 0;
+                for (int j = NW - 1; j >= LB; --j)
+                    if ((wb >> (j - LB)) & 1u) b[0] += hp[j];
 #pragma unroll
-            for (int c = 0; c < CPL; c += 2) {
-                const double ea = a + (b[c] + ql[c >> 1].x), eb = a + (b[c + 1] + ql[c >> 1].y);
-                if (ea < e1) {  // c ascending within the lane: strict '<' keeps the smallest index
-                    e1 = ea;
-                    i1 = c;
+                for (int c = 1; c < CPL; ++c) b[c] = b[c & (c - 1)] + hp[mp_ctz(c)];
+                double e1 = INFINITY;
+                unsigned i1 = 0;
+#pragma unroll
+                for (int c = 0; c < CPL; c += 2) {
+                    const double ea = a + (b[c] + ql[c >> 1].x), eb = a + (b[c + 1] + ql[c >> 1].y);
+                    if (ea < e1) {  // c ascending within the lane: strict '<' keeps the smallest index
+                        e1 = ea;
+                        i1 = c;
+                    }
+                    if (eb < e1) {
+                        e1 = eb;
+                        i1 = c + 1;
+                    }
                 }
-                if (eb < e1) {
-                    e1 = eb;
-                    i1 = c + 1;
+                i1 |= (ts << NL) | (lane << LB);
+                // lexicographic (e, index) minimum over the lanes.  Every e is positive (the offsets), so its bit pattern
+                // orders like its value: minimum of the high words, then of the low words among the lanes that hold it,
+                // then of the indices among those -- three warp reductions instead of five shuffle rounds.
+                const unsigned ehi = (unsigned)__double2hiint(e1), elo = (unsigned)__double2loint(e1);
+                const unsigned mhi = __reduce_min_sync(0xffffffffu, ehi);
+                const unsigned mlo = __reduce_min_sync(0xffffffffu, ehi == mhi ? elo : 0xffffffffu);
+                const bool tie = ehi == mhi && elo == mlo;
+                const unsigned mi = __reduce_min_sync(0xffffffffu, tie ? i1 : 0xffffffffu);
+                const double em = __hiloint2double((int)mhi, (int)mlo);
+                if (em < bestE || (em == bestE && mi < bestI)) {
+                    bestE = em;
+                    bestI = mi;
                 }
-            }
-            i1 |= (ts << NL) | (lane << LB);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const double e2 = mp_shfl(e1, (int)(lane ^ o));
-                const unsigned i2 = __shfl_xor_sync(0xffffffffu, i1, o);
-                if (e2 < e1 || (e2 == e1 && i2 < i1)) {
-                    e1 = e2;
-                    i1 = i2;
-                }
-            }
-            if (e1 < bestE || (e1 == bestE && i1 < bestI)) {
-                bestE = e1;
-                bestI = i1;
             }
         }
-    }
-    if (!outN) {
-        if (lane == 0) ws.best[p] = (uint64_t)bestI;
-        return;
-    }
-    // S7: N* and E(N*) = 1/2 d^T M d from the definition (Eq. (C1)); lane i holds dot i, d goes through shared memory
-    int32_t Ni = 0;
-    double di = 0.0;
-    if (lane < N) {
-        Ni = base_i + (int32_t)((bestI >> (N - 1 - lane)) & 1u);
-        di = (double)Ni - nc_i;
-        sd[wid][lane] = di;
-    }
-    __syncwarp();
-    const int li = lane < N ? lane : 0;
-    double row = 0.0;
+        if (!outN) {
+            if (lane == 0) ws.best[p] = (uint64_t)bestI;
+            __syncwarp();
+            continue;
+        }
+        // S7: N* and E(N*) = 1/2 d^T M d from the definition (Eq. (C1)); lane i holds dot i and row i of M
+        int32_t Ni = 0;
+        double di = 0.0;
+        if (lane < (unsigned)N) {
+            Ni = base_i + (int32_t)((bestI >> (N - 1 - lane)) & 1u);
+            di = (double)Ni - nc_i;
+            sd[wid][lane] = di;
+        }
+        __syncwarp();
+        double row = 0.0;
 #pragma unroll
-    for (int j = 0; j < N; ++j) row = fma(sM[li][j], sd[wid][j], row);
-    double E = di * row;  // lanes >= N hold di = 0
+        for (int j = 0; j < N; ++j) row = fma(Mrow[j], sd[wid][j], row);
+        double E = di * row;  // lanes >= N hold di = 0
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) E += mp_shfl(E, (int)(lane ^ o));
-    if (lane < N) outN[p * N + lane] = Ni;
-    if (lane == 0) outE[p] = 0.5 * E;
+        for (int o = 16; o > 0; o >>= 1) E += mp_shfl(E, (int)(lane ^ o));
+        if (lane < (unsigned)N) outN[p * N + lane] = Ni;
+        if (lane == 0) outE[p] = 0.5 * E;
+        __syncwarp();  // sIn / sd are rewritten by the next iteration
+    }
+}
+
+template <int NH, int NU, int NW>
+cudaError_t launch_finish(const QaDevModel *d_model, QaWorkspace ws, int32_t *d_N, double *d_E, int sm_count, cudaStream_t stream)
+{
+    int per_sm = 0;
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_finish_kernel<NH, NU, NW>, MF_THREADS, 0);
+    if (err != cudaSuccess) return err;
+    if (per_sm < 1) per_sm = 1;
+    int64_t grid = (int64_t)sm_count * per_sm;
+    const int64_t need = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
+    if (grid > need) grid = need;
+    return qa_launch_pdl(qa_minplus_finish_kernel<NH, NU, NW>, dim3((unsigned)grid), dim3(MF_THREADS), stream, d_model, ws, d_N,
+                         d_E);
 }
 
 template <int NH, int NU, int NW, int PX, int MINB>
@@ -631,9 +664,7 @@ cudaError_t launch_mp(const QaDevModel *d_model, const double *QLhost, QaWorkspa
     if (err != cudaSuccess) return err;
     qa_plan_add("qa_minplus_finish_kernel");
     qa_timing_mark(stream);
-    const int64_t fblocks = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
-    return qa_launch_pdl(qa_minplus_finish_kernel<NH, NU, NW>, dim3((unsigned)fblocks), dim3(MF_THREADS), stream, d_model, ws,
-                         d_N, d_E);
+    return launch_finish<NH, NU, NW>(d_model, ws, d_N, d_E, sm_count, stream);
 }
 
 }  // namespace
@@ -655,9 +686,7 @@ cudaError_t launch_mp_pruned(const QaDevModel *d_model, const double *QLhost, Qa
     if (err != cudaSuccess) return err;
     qa_plan_add("qa_minplus_finish_kernel");
     qa_timing_mark(stream);
-    const int64_t fblocks = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
-    return qa_launch_pdl(qa_minplus_finish_kernel<NH, 4, 4>, dim3((unsigned)fblocks), dim3(MF_THREADS), stream, d_model, ws, d_N,
-                         d_E);
+    return launch_finish<NH, 4, 4>(d_model, ws, d_N, d_E, sm_count, stream);
 }
 
 // d_N == nullptr: the finish kernel only stores the winning index (ws.best) and the caller runs qa_finalize_kernel.

@@ -126,7 +126,7 @@ def test_config4_open_grid16_default(api, W, H):
     """n = 16, 2^16 candidates per pixel: the hot kernel (NL = 8, NH = 8), QP pixels included."""
     w = wl.config4(W, H)
     rep, g, o = check(api, w, algorithm="default")
-    assert g["plan"][0] == ["qa_prologue_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"]
+    assert g["plan"][0] == ["qa_prologue_lanes_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"]
     assert g["stats"]["n_candidates_scored"] == w.P * 65536
 
 
@@ -139,8 +139,8 @@ def test_walk_variants_agree(api, n, P):
     w = wl.random_open(n, n, P, seed=200 + n)
     ref = None
     plans = {0: ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"],
-             1: ["qa_prologue_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"],
-             2: ["qa_prologue_kernel", "qa_minplus_pruned_kernel", "qa_minplus_finish_kernel"]}
+             1: ["qa_prologue_lanes_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"],
+             2: ["qa_prologue_lanes_kernel", "qa_minplus_pruned_kernel", "qa_minplus_finish_kernel"]}
     for variant in (0, 1, 2):
         rep, g, o = check(api, w, variant=variant, algorithm="default")
         assert g["plan"][0] == plans[variant]
@@ -350,7 +350,7 @@ def test_thermal_sum_product_kernel(api, n, P):
     EC = 0.5 * np.diag(M).min()
     for kT_over_EC in (0.3, max(0.05, 1.05 * gsum / 600.0 / EC)):
         Nm, o = check_thermal(api, w, kT_over_EC, algorithm="default")
-        assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_sp_kernel"]
+        assert api.last_launch_plan()[0] == ["qa_prologue_lanes_kernel", "qa_thermal_sp_kernel"]
         m0 = api.Model(w.C_dd, w.C_gd, walk_variant=0)
         r0 = m0.thermal(torch.from_numpy(w.Vg).cuda(), kT_over_EC * EC)
         assert api.last_launch_plan()[0][1].startswith("qa_thermal_gray_kernel")
@@ -367,7 +367,7 @@ def test_thermal_sum_product_full_size_sample(api):
     om = oracle.Model(w.C_dd, w.C_gd)
     kT = 0.05 * om.EC
     r = m.thermal(torch.from_numpy(w.Vg).cuda(), kT)
-    assert api.last_launch_plan()[0] == ["qa_prologue_kernel", "qa_thermal_sp_kernel"]
+    assert api.last_launch_plan()[0] == ["qa_prologue_lanes_kernel", "qa_thermal_sp_kernel"]
     sel = np.sort(np.random.default_rng(1).choice(w.P, size=300, replace=False))
     o = om.thermal(w.Vg[sel], kT)
     assert np.abs(r["Nmean"].cpu().numpy()[sel] - o["Nmean"]).max() <= 1e-9 * max(1.0, np.abs(o["Nmean"]).max())
