@@ -225,12 +225,12 @@ def run_ours(args, rank, world, local_rank):
     if rank != 0:
         return
 
-    # ---- opt-in exact pruning (qa_set_walk_variant(2)): same charge maps, fewer candidates scored explicitly; reported
-    # beside the headline, never instead of it
-    pruned = None
-    if args.workload == "config4":
+    # ---- opt-in variants, reported beside the headline, never instead of it: exact pruning (qa_model_set_walk_variant(2):
+    # same charge maps, fewer candidates scored explicitly) and the mixed-precision walk (variant 3: every candidate bounded
+    # from below in fp32 with directed rounding, the survivors re-scored in fp64: bit-identical N and E)
+    def time_variant(variant, note):
         for m_ in models:
-            m_.set_walk_variant(2)
+            m_.set_walk_variant(variant)
         try:
             for _ in range(3):
                 step()
@@ -243,13 +243,27 @@ def run_ours(args, rank, world, local_rank):
             torch.cuda.synchronize()
             tp = np.array([a.elapsed_time(b) for a, b in evp])
             ktp = api.kernel_times(models[0], Vgs[0], steps=args.steps, flush=flush)
-            pruned = {"ms_per_step": float(tp.mean()), "ms_per_step_median": float(np.median(tp)),
-                      "candidates_covered_per_s": cand_step / (float(tp.mean()) * 1e-3), "kernel_times_ms": ktp,
-                      "note": "qa_set_walk_variant(2): high patterns excluded by a rigorous lower bound are not walked; "
-                              "identical N and E (tests/test_gpu_parity.py)"}
+            return {"ms_per_step": float(tp.mean()), "ms_per_step_median": float(np.median(tp)),
+                    "candidates_covered_per_s": cand_step / (float(tp.mean()) * 1e-3), "kernel_times_ms": ktp, "note": note}
         finally:
             for m_ in models:
                 m_.set_walk_variant(1)
+
+    pruned = mixed = None
+    if args.workload == "config4":
+        pruned = time_variant(2, "qa_model_set_walk_variant(2): high patterns excluded by a rigorous lower bound are not walked; "
+                                 "identical N and E (tests/test_gpu_parity.py)")
+        mixed = time_variant(3, "qa_model_set_walk_variant(3): pass 1 bounds every candidate from below in fp32 (directed rounding), "
+                                "pass 2 re-scores the survivors in fp64: N and E bit-identical to the fp64 walk")
+        kw32 = mixed["kernel_times_ms"].get("qa_minplus_walk32_kernel", 0.0)
+        if kw32 > 0:
+            sm_count_ = torch.cuda.get_device_properties(dev).multi_processor_count
+            peak32 = sm_count_ * 128 * 1965.0e6
+            ops32 = 1.5 * wls[0].P * (2 ** wls[0].n_dot)       # 1 FADD + 1/2 VIMNMX3 per candidate
+            mixed["roofline"] = {"bound": "alu", "kernel": "qa_minplus_walk32_kernel", "achieved": ops32 / (kw32 * 1e-3) / 1e9,
+                                 "peak": peak32 / 1e9, "unit": "FP32/INT32 Ginst/s", "frac": ops32 / (kw32 * 1e-3) / peak32,
+                                 "ops_per_candidate": 1.5,
+                                 "peak_source": f"derived: {sm_count_} SMs x 128 FP32 lanes x 1965 MHz (DESIGN.md section 6)"}
 
     # ---- per-kernel share of the step: CUDA events between the kernels (separate pass, same launch configuration) --
     kt = api.kernel_times(models[0], Vgs[0], steps=args.steps, flush=flush)
@@ -312,7 +326,7 @@ def run_ours(args, rank, world, local_rank):
             "pixels_per_s": world * px_step / (ms_per_step * 1e-3), "diagram_ms": ms_per_step,
             "ms_per_step_min": float(times.min()), "ms_per_step_median": float(np.median(times)),
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-            "kernels_per_step": plan, "clocks": clocks, "pruned_variant": pruned,
+            "kernels_per_step": plan, "clocks": clocks, "pruned_variant": pruned, "mixed_precision_variant": mixed,
             "parity": parity, "secondary": secondary,
             "paper_context": "paper: same diagram shape in < 1 s on a GTX 1080 Ti via JAX (PAPER.md L7, L498)"}
     print(json.dumps(line), flush=True)

@@ -26,7 +26,9 @@ QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernel
 /* Kernel selection of ONE model (cross-check aid; the results are identical): 0 = the three-kernel path with the
  * exact-compare walk / the generic enumeration for every n_dot, 1 (default) = the production dispatch of DESIGN.md
  * section 5, 2 = as 1, but the open default search of n_dot >= 13 skips the high patterns a rigorous lower bound excludes
- * (same arg min; fewer candidates are scored explicitly).  Stored in the model (atomically); calls already enqueued are
+ * (same arg min; fewer candidates are scored explicitly), 3 = as 1, but pass 1 of that search bounds every candidate in fp32
+ * (packed adds, explicit error bound) and the fp64 pass 2 re-scores the threads the bound cannot exclude: charge map and
+ * energies bit-identical to variant 1 (the "fp32 walk, fp64 re-score" path of SURVEY 8(f) NEXT-4).  Stored in the model (atomically); calls already enqueued are
  * not affected.  Returns QA_ERR_INVALID_ARG for any other value.  The initial value of every model comes from the
  * environment variable QA_WALK_VARIANT (default 1). */
 QA_API qa_status qa_model_set_walk_variant(qa_model *model, int variant);

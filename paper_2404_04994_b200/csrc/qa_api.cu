@@ -186,7 +186,7 @@ int initial_walk_variant()
 {
     const char *e = std::getenv("QA_WALK_VARIANT");
     const int v = e ? std::atoi(e) : 1;
-    return (v < 0 || v > 2) ? 1 : v;
+    return (v < 0 || v > 3) ? 1 : v;
 }
 
 // A model (batch) belongs to the device that was current when it was created.
@@ -280,8 +280,11 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd
     if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && variant != 0 && m->is_z) {
         const bool fuse = m->ns == 0;  // S7 runs inside the finish kernel: no finalize launch
-        QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count,
-                                       variant == 2, stream));
+        if (variant == 3)  // mixed precision: fp32 lower-bound pass 1, fp64 exact pass 2 (same charge map, bit for bit)
+            QA_CUDA(qa_launch_minplus_walk32(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count, stream));
+        else
+            QA_CUDA(qa_launch_minplus_walk(m->dev, n, m->host.QL, ws, fuse ? d_N : nullptr, d_E, m->sm_count,
+                                           variant == 2, stream));
         timing_mark(stream);
         if (fuse) return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && closed && n > QA_WALK_NL && variant != 0) {
@@ -732,7 +735,7 @@ qa_status qa_set_kernel_timing(int enable)
 
 qa_status qa_model_set_walk_variant(qa_model *m, int variant)
 {
-    if (!m || variant < 0 || variant > 2) return QA_ERR_INVALID_ARG;
+    if (!m || variant < 0 || variant > 3) return QA_ERR_INVALID_ARG;
     m->walk_variant.store(variant, std::memory_order_relaxed);
     return QA_OK;
 }

@@ -472,7 +472,7 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_pruned_kernel(con
 template <int NH, int NU, int NW>
 __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaDevModel *__restrict__ mdl,
                                                                        QaWorkspace ws, int32_t *__restrict__ outN,
-                                                                       double *__restrict__ outE)
+                                                                       double *__restrict__ outE, unsigned slack)
 {
     constexpr int NL = NU + NW;
     constexpr int N = NL + NH;
@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaD
         const double *__restrict__ h = sIn[wid];
         const double e0 = h[N];
         const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
-        const unsigned wmask = __ballot_sync(0xffffffffu, lane < (unsigned)WPP && r.x <= H + 2u);  // warps that may hold the argmin
+        const unsigned wmask = __ballot_sync(0xffffffffu, lane < (unsigned)WPP && r.x <= H + slack);  // warps that may hold the argmin
 
         // thread-independent offsets, as pass 1 formed them (j ascending)
         double offw = EC, offu = 0.0;
@@ -630,7 +630,8 @@ __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaD
 }
 
 template <int NH, int NU, int NW>
-cudaError_t launch_finish(const QaDevModel *d_model, QaWorkspace ws, int32_t *d_N, double *d_E, int sm_count, cudaStream_t stream)
+cudaError_t launch_finish(const QaDevModel *d_model, QaWorkspace ws, int32_t *d_N, double *d_E, int sm_count, cudaStream_t stream,
+                          unsigned slack = 2u)
 {
     int per_sm = 0;
     cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_finish_kernel<NH, NU, NW>, MF_THREADS, 0);
@@ -640,7 +641,7 @@ cudaError_t launch_finish(const QaDevModel *d_model, QaWorkspace ws, int32_t *d_
     const int64_t need = (ws.P + MF_THREADS / 32 - 1) / (MF_THREADS / 32);
     if (grid > need) grid = need;
     return qa_launch_pdl(qa_minplus_finish_kernel<NH, NU, NW>, dim3((unsigned)grid), dim3(MF_THREADS), stream, d_model, ws, d_N,
-                         d_E);
+                         d_E, slack);
 }
 
 template <int NH, int NU, int NW, int PX, int MINB>
@@ -713,4 +714,20 @@ cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const doubl
         default: return cudaErrorInvalidValue;
     }
 #undef MP_CALL
+}
+
+// Pass 2 + S7 on records another pass 1 wrote (qa_kernels_minplus32.cu): `slack` = how far, in units of the record key, a
+// thread's bound may lie above the pixel minimum and still hold the argmin.
+cudaError_t qa_launch_minplus_finish(const QaDevModel *d_model, int n, QaWorkspace ws, int32_t *d_N, double *d_E, unsigned slack,
+                                     int sm_count, cudaStream_t stream)
+{
+    qa_plan_add("qa_minplus_finish_kernel");
+    qa_timing_mark(stream);
+    switch (n) {
+        case 13: return launch_finish<5, 4, 4>(d_model, ws, d_N, d_E, sm_count, stream, slack);
+        case 14: return launch_finish<6, 4, 4>(d_model, ws, d_N, d_E, sm_count, stream, slack);
+        case 15: return launch_finish<7, 4, 4>(d_model, ws, d_N, d_E, sm_count, stream, slack);
+        case 16: return launch_finish<8, 4, 4>(d_model, ws, d_N, d_E, sm_count, stream, slack);
+        default: return cudaErrorInvalidValue;
+    }
 }

@@ -165,13 +165,18 @@ def full_size_report(api, oracle, wl, torch, strict=False, config5_members=256, 
         om = oracle.Model(w.C_dd, w.C_gd)
         o = om.ground_state(w.Vg, n_threads=nt)
         rs = []
-        for variant in (1, 2, 0):
+        for variant in (1, 2, 0, 3):
             g = _gpu(api, torch, w, variant=variant)
             rs.append(compare(g["N"], g["E"], o, om.EC, g["xcont"], strict=strict))
+            if variant == 1:
+                g1 = g
+        r_mixed_equal = bool(np.array_equal(g["N"], g1["N"]) and np.array_equal(g["E"], g1["E"]))
         r = dict(rs[0])
         for k in ("mismatch", "excused_near_tie", "unexcused", "E_out_of_tolerance"):
             r[k + "_all_variants"] = int(sum(x[k] for x in rs))
-        r.update(algorithms="default; walk variants 1 (min-plus), 2 (pruned), 0 (exact-compare walk), each vs the oracle",
+        r["mixed_precision_walk_bit_identical_to_fp64_walk"] = r_mixed_equal
+        r.update(algorithms="default; walk variants 1 (min-plus), 2 (pruned), 0 (exact-compare walk), 3 (fp32 lower-bound pass + "
+                            "fp64 re-score), each vs the oracle",
                  oracle_s=round(time.perf_counter() - t0, 2))
         rep["config4"] = r
     if 5 in configs:
