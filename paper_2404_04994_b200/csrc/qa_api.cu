@@ -215,7 +215,10 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
     uint64_t *tt = static_cast<uint64_t *>(take(Pz * 8));
     uint64_t *be = static_cast<uint64_t *>(take(Pz * 8));
     double *e0 = static_cast<double *>(take(Pz * 8));
-    uint2 *rec = static_cast<uint2 *>(take(n >= 13 ? Pz * 8 * ((size_t)1 << (n - 13)) : 0));
+    // records of the min-plus walk (n >= 13: 8 bytes per warp of a pixel) or of the closed walk (n >= 9: 16 bytes per block)
+    size_t rec_bytes = n >= 13 ? Pz * 8 * ((size_t)1 << (n - 13)) : 0;
+    if (n > QA_WALK_NL && rec_bytes < Pz * 16 * (size_t)QA_CLOSED_MAXB) rec_bytes = Pz * 16 * (size_t)QA_CLOSED_MAXB;
+    uint2 *rec = static_cast<uint2 *>(take(rec_bytes));
     unsigned long long *counter = static_cast<unsigned long long *>(take(256));
     if (ws) {
         ws->h = h;
@@ -226,6 +229,7 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
         ws->best = be;
         ws->e0 = e0;
         ws->rec = rec;
+        ws->rec2 = reinterpret_cast<double2 *>(rec);
         ws->counter = counter;
         ws->P = P;
     }
@@ -289,8 +293,12 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
         if (fuse) return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && closed && n > QA_WALK_NL && variant != 0) {
         // closed default set of a larger array: only the C(n, k) states with the right total are visited (NEXT-3)
-        QA_CUDA(qa_launch_closed_walk(m->dev, n, m->walk, ws, a, d_stats, m->sm_count, stream));
+        int nb = 0;
+        QA_CUDA(qa_launch_closed_walk(m->dev, n, m->walk, ws, a, m->sm_count, stream, &nb));
         timing_mark(stream);
+        QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream, nb, N_hat));
+        timing_mark(stream);
+        return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && !closed) {
         QA_CUDA(qa_launch_walk(m->dev, n, m->walk, ws, d_stats, m->sm_count, stream));
         timing_mark(stream);

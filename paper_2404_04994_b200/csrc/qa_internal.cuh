@@ -10,6 +10,7 @@ constexpr int QA_MAXN = 16;  // dots
 constexpr int QA_MAXG = 64;  // gates
 constexpr int QA_WALK_NL = 8;  // low bits walked per thread by the static Gray walk (2^8 candidates per thread)
 constexpr int QA_FUSED_MAXN = 8; // largest n of the one-kernel path (qa_kernels_fused.cu)
+constexpr int QA_CLOSED_MAXB = 16; // most blocks of high patterns per pixel in the closed walk (qa_kernels_closed.cu)
 constexpr int QA_PAIR_NL = 10; // low bits covered by the model's pair-energy table QL (min-plus walk: NL <= 10)
 
 // Pixel-independent model constants in device global memory (one per qa_model).
@@ -53,6 +54,7 @@ struct QaWorkspace {
     double *e0;       // [P]     E(base) = 1/2 (base - N_c)^T M (base - N_c) >= 0, the energy of the base point
     unsigned long long *counter;  // work counter of the pruned min-plus walk (zeroed by the prologue kernel)
     uint2 *rec;       // [P][2^(n-13)]  min-plus walk: per warp of the pixel (min of L over its lanes, ballot of lanes near it)
+    double2 *rec2;    // [P][nb]        closed walk (same storage as rec): per block of high patterns (best energy, its index)
     int64_t P;
 };
 
@@ -84,7 +86,7 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
 cudaError_t qa_launch_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, qa_stats *d_stats,
                            int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_closed_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, QaCallArgs args,
-                                  qa_stats *d_stats, int sm_count, cudaStream_t stream);
+                                  int sm_count, cudaStream_t stream, int *nb_out);
 cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
                                    double *d_E, int sm_count, int pruned, cudaStream_t stream);
 cudaError_t qa_launch_minplus_finish(const QaDevModel *d_model, int n, QaWorkspace ws, int32_t *d_N, double *d_E, unsigned slack,
@@ -101,8 +103,10 @@ cudaError_t qa_launch_thermal(const QaDevModel *d_model, int n, QaWorkspace ws, 
                               double expect_cand, double *d_Nmean, double *d_Emin, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_thermal_sp(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, double kT,
                                  double *d_Nmean, double *d_Emin, int sm_count, cudaStream_t stream);
+// closed_nb > 0: the winner of a pixel is the lexicographic minimum of its closed_nb records ws.rec2 (closed walk); N_hat is
+// then read for the scored-candidate counter
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
-                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream);
+                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream, int closed_nb = 0, int N_hat = 0);
 cudaError_t qa_launch_sensor_response(const qa_sensor_params *params, int ns, const double *d_Vs, int64_t P, int64_t W,
                                       double *d_S, double *d_G, double *d_partial, cudaStream_t stream);
 size_t qa_sensor_workspace_bytes_impl(int64_t P, int ns);

@@ -10,13 +10,18 @@
 // and the admissible (u, w) of a thread are those with popcount(u) + popcount(w) = kr := k - popcount(t): for every u the
 // popcount class kr - popcount(u) of the 4-bit patterns w (1, 4, 6, 4, 1 members).  The loop over u and the members of each
 // class are unrolled, so every register and table index is static (the table is a kernel parameter: constant bank); what is
-// dynamic is only WHICH class a thread walks for a given u.  To keep that choice uniform inside a warp the 2^NH patterns
-// t are handed to the threads sorted by popcount (colex rank inside a class), so at most two or three classes meet in a warp.
+// dynamic is only WHICH class a thread walks for a given u.  The work of a pattern follows C(8, k - popcount(t)) (70 states
+// for the middle class, 1 for the outer ones), so the patterns are cut into BLOCKS of up to 32 of (nearly) one popcount
+// (host table CwBlocks) and a WORK ITEM is (pixel, block): every warp is an independent worker over the items
+// gw, gw + #warps, ... -- no CTA barrier, lanes of a warp walk the same class, light and heavy blocks mix over the grid.
 // Per candidate: 2 DADD + 1 DSETP (the energy itself is compared, exactly; ascending index order + strict '<' gives the
-// lexicographically smallest N among bitwise ties, reading R6); the winner over the threads of the pixel is a
-// lexicographic (e, index) minimum.  E(N*) is recomputed from the definition by qa_finalize_kernel.
+// lexicographically smallest N among bitwise ties, reading R6); the warp's winner (lexicographic (e, index) minimum, three
+// warp reductions on a monotone integer key of the energy) is one 16-byte record per item, and qa_finalize_kernel takes the
+// lexicographic minimum of a pixel's records before it decodes N* and recomputes E(N*) from the definition.
 //
 // Works for any SPD c_dd (no positivity offsets are used).  Index convention as in qa_kernels_walk.cu.
+#include <cstring>
+
 #include "qa_internal.cuh"
 
 namespace {
@@ -94,79 +99,81 @@ struct CwLoop<16> {
     }
 };
 
+// blocks of high patterns: up to 32 patterns per block, a class of >= 16 patterns starts its own block
+struct CwBlocks {
+    int nb;
+    unsigned mask[QA_CLOSED_MAXB];
+    unsigned char t[QA_CLOSED_MAXB][32];
+};
+
+// monotone map double -> uint64 (orders like the values, negative ones included)
+__device__ __forceinline__ unsigned long long cw_key(double e)
+{
+    const unsigned long long b = (unsigned long long)__double_as_longlong(e);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double cw_unkey(unsigned long long k)
+{
+    const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)b);
+}
+
 template <int NH>
-__global__ void __launch_bounds__(CW_THREADS) qa_closed_walk_kernel(const QaDevModel *__restrict__ mdl,
-                                                                    const __grid_constant__ QaWalkTable tab, QaWorkspace ws,
-                                                                    QaCallArgs args, qa_stats *stats)
+__global__ void __launch_bounds__(CW_THREADS, 3) qa_closed_walk_kernel(const QaDevModel *__restrict__ mdl,
+                                                                       const __grid_constant__ QaWalkTable tab,
+                                                                       const __grid_constant__ CwBlocks blk, QaWorkspace ws,
+                                                                       QaCallArgs args)
 {
     constexpr int NL = QA_WALK_NL;
     constexpr int N = NL + NH;
-    constexpr int TPP = 1 << NH;            // threads per pixel
-    constexpr int PPB = CW_THREADS / TPP;   // pixels per CTA
-    constexpr int WPP = TPP > 32 ? TPP / 32 : 1;
+    constexpr int WARPS = CW_THREADS / 32;
     static_assert(NL == 8 && NH >= 1 && NH <= 8, "low bits = two groups of four");
-    __shared__ double sIn[PPB][N + 1];
-    __shared__ int sK[PPB];
-    __shared__ unsigned char sPerm[TPP];
-    __shared__ double sE[CW_THREADS / 32];
-    __shared__ unsigned sI[CW_THREADS / 32];
-
-    const unsigned r = threadIdx.x & (TPP - 1);
-    const int slot = threadIdx.x >> NH;
+    __shared__ double sIn[WARPS][N + 1];
+    const unsigned lane = threadIdx.x & 31u;
+    const int wid = threadIdx.x >> 5;
     const int64_t P = ws.P;
-    // patterns sorted by popcount, colex rank inside a class: rank(x) = #(popcount < pc) + sum_i C(p_i, i), p_1 < p_2 < ...
-    if (threadIdx.x < TPP) {
-        const unsigned x = threadIdx.x;
-        const int pc = __popc(x);
-        int rank = 0;
-        for (int c = 0; c < pc; ++c) rank += cw_binom(NH, c);
-        int i = 0;
-        for (int b = 0; b < NH; ++b)
-            if ((x >> b) & 1u) rank += cw_binom(b, ++i);
-        sPerm[rank] = (unsigned char)x;
-    }
-    __syncthreads();
-    const unsigned t = sPerm[r];
-    double v[NL];
-#pragma unroll
-    for (int j = 0; j < NL; ++j) v[j] = mdl->VT[t * NL + j];
-    const double QH = mdl->QHT[t];
+    const int NB = blk.nb;
+    const int64_t items = P * NB;
+    const bool small = items < 0x7fffffff;  // 32-bit division of the item index (a 64-bit one costs ~100 instructions)
+    auto pixel_of = [&](int64_t item) -> int64_t {
+        return small ? (int64_t)((unsigned)item / (unsigned)NB) : item / NB;
+    };
+    const int64_t gw = (int64_t)wid * gridDim.x + blockIdx.x;  // consecutive warps sit in different CTAs
+    const int64_t tw = (int64_t)gridDim.x * WARPS;
     qa_pdl_launch_dependents();
-    qa_pdl_wait();  // model constants above; h, e0, base come from the prologue kernel
+    qa_pdl_wait();  // h, e0, base come from the prologue kernel
 
-    // persistent: a CTA walks pixel groups blockIdx.x, blockIdx.x + gridDim.x, ... (the per-thread tables above are loaded once)
-    const int64_t groups = (P + PPB - 1) / PPB;
-    for (int64_t grp = blockIdx.x; grp < groups; grp += gridDim.x) {
-        const int64_t p0 = grp * PPB;
-        if (threadIdx.x < PPB) sK[threadIdx.x] = 0;
-        __syncthreads();  // also: the previous group's sIn / sE / sI have been read
-        for (int e = threadIdx.x; e < PPB * (N + 1); e += CW_THREADS) {
-            const int s = e / (N + 1), i = e % (N + 1);
-            int64_t p = p0 + s;
-            if (p >= P) p = P - 1;
-            if (i < N) {
-                sIn[s][i] = __ldg(ws.h + (int64_t)i * P + p);
-                atomicAdd(&sK[s], ws.base[(int64_t)i * P + p]);
-            } else {
-                sIn[s][N] = __ldg(ws.e0 + p);
-            }
-        }
-        __syncthreads();
-        const int64_t p = p0 + slot;
-        const bool live = p < P;
-        const int k = args.N_hat - sK[slot];  // ones to place
+    // inputs of an item's pixel, one value per lane, requested one item ahead
+    double in_v = 0.0;
+    int in_base = 0;
+    auto request = [&](int64_t item) {
+        if (item >= items) return;
+        const int64_t p = pixel_of(item);
+        if (lane <= (unsigned)N) in_v = lane < (unsigned)N ? __ldg(ws.h + (int64_t)lane * P + p) : __ldg(ws.e0 + p);
+        in_base = lane < (unsigned)N ? ws.base[(int64_t)lane * P + p] : 0;
+    };
+    request(gw);
+    for (int64_t item = gw; item < items; item += tw) {
+        const int64_t p = pixel_of(item);
+        const int b = (int)(item - p * NB);
+        const int k = args.N_hat - __reduce_add_sync(0xffffffffu, in_base);  // ones to place
+        if (lane <= (unsigned)N) sIn[wid][lane] = in_v;
+        __syncwarp();
+        request(item + tw);
+        const bool active = (blk.mask[b] >> lane) & 1u;
+        const unsigned t = blk.t[b][lane];
         const int kr = k - __popc(t);
-
         double best = INFINITY;
         unsigned bi = 0xffffffffu;
-        if (kr >= 0 && kr <= NL) {
+        if (active && kr >= 0 && kr <= NL) {
+            const double *__restrict__ h = sIn[wid];
             double hp[NL];
 #pragma unroll
-            for (int j = 0; j < NL; ++j) hp[j] = sIn[slot][N - 1 - j] + v[j];
-            double be = sIn[slot][N] + QH;
+            for (int j = 0; j < NL; ++j) hp[j] = h[N - 1 - j] + __ldg(mdl->VT + t * NL + j);
+            double be = h[N] + __ldg(mdl->QHT + t);
 #pragma unroll
             for (int jh = 0; jh < NH; ++jh)
-                if ((t >> jh) & 1u) be += sIn[slot][N - 1 - NL - jh];
+                if ((t >> jh) & 1u) be += h[N - 1 - NL - jh];
             double B[16], A[16];
             B[0] = 0.0;
             A[0] = be;
@@ -178,75 +185,78 @@ __global__ void __launch_bounds__(CW_THREADS) qa_closed_walk_kernel(const QaDevM
             CwLoop<0>::run(tab, B, A, kr, best, bi);
             if (bi != 0xffffffffu) bi |= t << NL;
         }
-
-        // lexicographic (e, index) minimum over the threads of the pixel
-        constexpr int W = TPP < 32 ? TPP : 32;
-#pragma unroll
-        for (int o = W / 2; o > 0; o >>= 1) {
-            const double e2 = __shfl_xor_sync(0xffffffffu, best, o);
-            const unsigned i2 = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (e2 < best || (e2 == best && i2 < bi)) {
-                best = e2;
-                bi = i2;
-            }
+        // lexicographic (e, index) minimum over the lanes: minimum of the key's high word, then of its low word among the
+        // lanes that hold it, then of the index among those
+        const unsigned long long key = bi != 0xffffffffu ? cw_key(best) : ~0ull;
+        const unsigned khi = (unsigned)(key >> 32), klo = (unsigned)key;
+        const unsigned mhi = __reduce_min_sync(0xffffffffu, khi);
+        const unsigned mlo = __reduce_min_sync(0xffffffffu, khi == mhi ? klo : 0xffffffffu);
+        const unsigned mi = __reduce_min_sync(0xffffffffu, (khi == mhi && klo == mlo) ? bi : 0xffffffffu);
+        if (lane == 0) {
+            const double e = mi != 0xffffffffu ? cw_unkey(((unsigned long long)mhi << 32) | mlo) : INFINITY;
+            ws.rec2[item] = make_double2(e, __longlong_as_double((long long)(unsigned long long)mi));
         }
-        if (WPP > 1) {
-            const int wq = threadIdx.x >> 5;
-            if ((threadIdx.x & 31) == 0) {
-                sE[wq] = best;
-                sI[wq] = bi;
-            }
-            __syncthreads();
-            if (r == 0) {
-#pragma unroll
-                for (int q = 1; q < WPP; ++q) {
-                    const double e2 = sE[wq + q];
-                    const unsigned i2 = sI[wq + q];
-                    if (e2 < best || (e2 == best && i2 < bi)) {
-                        best = e2;
-                        bi = i2;
-                    }
-                }
-            }
-        }
-        if (live && r == 0) {
-            ws.best[p] = bi == 0xffffffffu ? ~0ull : (uint64_t)bi;
-            if (stats) qa_atomic_add64(&stats->n_candidates_scored, (int64_t)cw_binom(N, k));
-        }
+        __syncwarp();  // sIn is rewritten by the next iteration
     }
 }
 
 template <int NH>
-cudaError_t launch_cw(const QaDevModel *d_model, const QaWalkTable &tab, QaWorkspace ws, QaCallArgs args, qa_stats *d_stats,
-                      int sm_count, cudaStream_t stream)
+cudaError_t launch_cw(const QaDevModel *d_model, const QaWalkTable &tab, QaWorkspace ws, QaCallArgs args, int sm_count,
+                      cudaStream_t stream, int *nb_out)
 {
-    constexpr int PPB = CW_THREADS >> NH;
-    const int64_t groups = (ws.P + PPB - 1) / PPB;
+    // patterns by popcount (ascending value inside a class); a class of >= 16 patterns starts a new block
+    CwBlocks blk;
+    std::memset(&blk, 0, sizeof(blk));
+    int nb = 0, fill = 0;
+    for (int c = 0; c <= NH; ++c) {
+        if (cw_binom(NH, c) >= 16 && fill > 0) {
+            ++nb;
+            fill = 0;
+        }
+        for (int t = 0; t < (1 << NH); ++t) {
+            if (__builtin_popcount((unsigned)t) != c) continue;
+            if (fill == 32) {
+                ++nb;
+                fill = 0;
+            }
+            blk.t[nb][fill] = (unsigned char)t;
+            blk.mask[nb] |= 1u << fill;
+            ++fill;
+        }
+        if (cw_binom(NH, c) >= 16) {
+            ++nb;
+            fill = 0;
+        }
+    }
+    if (fill > 0) ++nb;
+    blk.nb = nb;
+    *nb_out = nb;
     int per_sm = 0;
     cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_closed_walk_kernel<NH>, CW_THREADS, 0);
     if (err != cudaSuccess) return err;
     if (per_sm < 1) per_sm = 1;
     int64_t grid = (int64_t)sm_count * per_sm;
-    if (grid > groups) grid = groups;
-    return qa_launch_pdl(qa_closed_walk_kernel<NH>, dim3((unsigned)grid), dim3(CW_THREADS), stream, d_model, tab, ws, args,
-                         d_stats);
+    const int64_t need = (ws.P * nb + CW_THREADS / 32 - 1) / (CW_THREADS / 32);
+    if (grid > need) grid = need;
+    return qa_launch_pdl(qa_closed_walk_kernel<NH>, dim3((unsigned)grid), dim3(CW_THREADS), stream, d_model, tab, blk, ws, args);
 }
 
 }  // namespace
 
+// *nb_out = records per pixel (ws.rec2[p * nb + b]) for qa_launch_finalize
 cudaError_t qa_launch_closed_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, QaCallArgs args,
-                                  qa_stats *d_stats, int sm_count, cudaStream_t stream)
+                                  int sm_count, cudaStream_t stream, int *nb_out)
 {
     qa_plan_add("qa_closed_walk_kernel");
     switch (n) {
-        case 9: return launch_cw<1>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 10: return launch_cw<2>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 11: return launch_cw<3>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 12: return launch_cw<4>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 13: return launch_cw<5>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 14: return launch_cw<6>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 15: return launch_cw<7>(d_model, tab, ws, args, d_stats, sm_count, stream);
-        case 16: return launch_cw<8>(d_model, tab, ws, args, d_stats, sm_count, stream);
+        case 9: return launch_cw<1>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 10: return launch_cw<2>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 11: return launch_cw<3>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 12: return launch_cw<4>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 13: return launch_cw<5>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 14: return launch_cw<6>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 15: return launch_cw<7>(d_model, tab, ws, args, sm_count, stream, nb_out);
+        case 16: return launch_cw<8>(d_model, tab, ws, args, sm_count, stream, nb_out);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -426,11 +426,35 @@ __global__ void __launch_bounds__(ENUM_THREADS) qa_enumerate_kernel(const QaDevM
 __global__ void __launch_bounds__(FIN_THREADS) qa_finalize_kernel(const QaDevModel *__restrict__ mdl,
                                                                   const double *__restrict__ Vg, QaWorkspace ws,
                                                                   int32_t *__restrict__ outN, double *__restrict__ outE,
-                                                                  double *__restrict__ outVs)
+                                                                  double *__restrict__ outVs, int closed_nb, int N_hat,
+                                                                  qa_stats *stats)
 {
     const int64_t p = blockIdx.x * (int64_t)FIN_THREADS + threadIdx.x;
-    qa_pdl_wait();  // ws.best comes from the candidate kernel launched just before
-    if (p >= ws.P) return;
+    qa_pdl_wait();  // ws.best / ws.rec2 come from the candidate kernel launched just before
+    const bool live = p < ws.P;
+    if (closed_nb > 0) {  // closed walk: lexicographic minimum of the pixel's records; C(n, k) states were scored
+        int64_t scored = 0;
+        if (live) {
+            double be = INFINITY;
+            uint64_t bi = ~0ull;
+            for (int b = 0; b < closed_nb; ++b) {
+                const double2 r = ws.rec2[p * closed_nb + b];
+                const uint64_t i2 = (uint64_t)(uint32_t)__double_as_longlong(r.y);
+                if (i2 != 0xffffffffull) qa_lexmin(be, bi, r.x, i2);
+            }
+            int k = N_hat;
+            const int n = mdl->n;
+            for (int i = 0; i < n; ++i) k -= ws.base[(int64_t)i * ws.P + p];
+            if (k >= 0 && k <= n) {
+                scored = 1;
+                for (int i = 1; i <= k; ++i) scored = scored * (n - k + i) / i;
+            }
+            qa_finalize_pixel(mdl, Vg, ws, p, bi, outN, outE, outVs);
+        }
+        if (stats) qa_warp_count(&stats->n_candidates_scored, scored);
+        return;
+    }
+    if (!live) return;
     qa_finalize_pixel(mdl, Vg, ws, p, ws.best[p], outN, outE, outVs);
 }
 
@@ -561,12 +585,12 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
 }
 
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
-                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream)
+                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream, int closed_nb, int N_hat)
 {
-    (void)d_stats;
     qa_plan_add("qa_finalize_kernel");
     const unsigned blocks = (unsigned)((ws.P + FIN_THREADS - 1) / FIN_THREADS);
-    return qa_launch_pdl(qa_finalize_kernel, dim3(blocks), dim3(FIN_THREADS), stream, d_model, d_Vg, ws, d_N, d_E, d_Vsensor);
+    return qa_launch_pdl(qa_finalize_kernel, dim3(blocks), dim3(FIN_THREADS), stream, d_model, d_Vg, ws, d_N, d_E, d_Vsensor,
+                         closed_nb, N_hat, d_stats);
 }
 
 cudaError_t qa_launch_fp64_probe(double *d_sink, int blocks, int threads, int iters, cudaStream_t stream)
