@@ -296,7 +296,8 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
         int nb = 0;
         QA_CUDA(qa_launch_closed_walk(m->dev, n, m->walk, ws, a, m->sm_count, stream, &nb));
         timing_mark(stream);
-        QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream, nb, N_hat));
+        QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream, nb, N_hat,
+                                   (m->ns == 0 && variant != 0) ? n : 0));
         timing_mark(stream);
         return QA_OK;
     } else if (alg == QA_ALG_DEFAULT && !closed) {
@@ -309,7 +310,8 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
         QA_CUDA(qa_launch_enumerate(m->dev, n, ws, a, expect, d_stats, stream));
         timing_mark(stream);
     }
-    QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream));
+    QA_CUDA(qa_launch_finalize(m->dev, d_Vg, ws, d_N, d_E, m->ns > 0 ? d_Vsensor : nullptr, d_stats, stream, 0, 0,
+                               (m->ns == 0 && variant != 0) ? n : 0));
     timing_mark(stream);
     return QA_OK;
 }

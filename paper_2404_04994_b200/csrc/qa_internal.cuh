@@ -54,7 +54,7 @@ struct QaWorkspace {
     double *e0;       // [P]     E(base) = 1/2 (base - N_c)^T M (base - N_c) >= 0, the energy of the base point
     unsigned long long *counter;  // work counter of the pruned min-plus walk (zeroed by the prologue kernel)
     uint2 *rec;       // [P][2^(n-13)]  min-plus walk: per warp of the pixel (min of L over its lanes, ballot of lanes near it)
-    double2 *rec2;    // [P][nb]        closed walk (same storage as rec): per block of high patterns (best energy, its index)
+    double2 *rec2;    // [nb][P]        closed walk (same storage as rec): per block of high patterns (best energy, its index)
     int64_t P;
 };
 
@@ -106,7 +106,8 @@ cudaError_t qa_launch_thermal_sp(const QaDevModel *d_model, int n, const double 
 // closed_nb > 0: the winner of a pixel is the lexicographic minimum of its closed_nb records ws.rec2 (closed walk); N_hat is
 // then read for the scored-candidate counter
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
-                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream, int closed_nb = 0, int N_hat = 0);
+                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream, int closed_nb = 0, int N_hat = 0,
+                               int n_lanes = 0);  // n_lanes = n_dot when the sixteen-lanes-per-pixel kernel may be used, else 0
 cudaError_t qa_launch_sensor_response(const qa_sensor_params *params, int ns, const double *d_Vs, int64_t P, int64_t W,
                                       double *d_S, double *d_G, double *d_partial, cudaStream_t stream);
 size_t qa_sensor_workspace_bytes_impl(int64_t P, int ns);

@@ -194,7 +194,7 @@ __global__ void __launch_bounds__(CW_THREADS, 3) qa_closed_walk_kernel(const QaD
         const unsigned mi = __reduce_min_sync(0xffffffffu, (khi == mhi && klo == mlo) ? bi : 0xffffffffu);
         if (lane == 0) {
             const double e = mi != 0xffffffffu ? cw_unkey(((unsigned long long)mhi << 32) | mlo) : INFINITY;
-            ws.rec2[item] = make_double2(e, __longlong_as_double((long long)(unsigned long long)mi));
+            ws.rec2[(int64_t)b * P + p] = make_double2(e, __longlong_as_double((long long)(unsigned long long)mi));
         }
         __syncwarp();  // sIn is rewritten by the next iteration
     }
@@ -243,7 +243,7 @@ cudaError_t launch_cw(const QaDevModel *d_model, const QaWalkTable &tab, QaWorks
 
 }  // namespace
 
-// *nb_out = records per pixel (ws.rec2[p * nb + b]) for qa_launch_finalize
+// *nb_out = records per pixel (ws.rec2[b * P + p]) for qa_launch_finalize
 cudaError_t qa_launch_closed_walk(const QaDevModel *d_model, int n, const QaWalkTable &tab, QaWorkspace ws, QaCallArgs args,
                                   int sm_count, cudaStream_t stream, int *nb_out)
 {

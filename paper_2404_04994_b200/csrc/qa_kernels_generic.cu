@@ -438,7 +438,7 @@ __global__ void __launch_bounds__(FIN_THREADS) qa_finalize_kernel(const QaDevMod
             double be = INFINITY;
             uint64_t bi = ~0ull;
             for (int b = 0; b < closed_nb; ++b) {
-                const double2 r = ws.rec2[p * closed_nb + b];
+                const double2 r = ws.rec2[(int64_t)b * ws.P + p];
                 const uint64_t i2 = (uint64_t)(uint32_t)__double_as_longlong(r.y);
                 if (i2 != 0xffffffffull) qa_lexmin(be, bi, r.x, i2);
             }
@@ -456,6 +456,85 @@ __global__ void __launch_bounds__(FIN_THREADS) qa_finalize_kernel(const QaDevMod
     }
     if (!live) return;
     qa_finalize_pixel(mdl, Vg, ws, p, ws.best[p], outN, outE, outVs);
+}
+
+// Finalize for 9..16 search dots without sensor dots, sixteen lanes per pixel (lane i <-> dot i): the thread-per-pixel kernel
+// above puts 10^4 pixels on 79 CTAs and each thread through n^2 dependent FMAs and n 64-bit divisions.  Here lane i decodes
+// its own digit of the winning mixed-radix index (suffix products of cnt by a shuffle scan), forms d_i = N_i - N_c,i and
+// row i of M d (j ascending, d_j by shuffle); E(N*) = 1/2 sum_i d_i (M d)_i is a four-step butterfly sum.
+__global__ void __launch_bounds__(256) qa_finalize_lanes_kernel(const QaDevModel *__restrict__ mdl, QaWorkspace ws,
+                                                                int32_t *__restrict__ outN, double *__restrict__ outE,
+                                                                int closed_nb, int N_hat, qa_stats *stats)
+{
+    __shared__ double sM[QA_MAXN * QA_MAXN];
+    const int n = mdl->n;
+    for (int e = threadIdx.x; e < n * n; e += 256) sM[e] = mdl->M[(e / n) * QA_MAXN + (e % n)];
+    __syncthreads();
+    qa_pdl_wait();  // ws.best / ws.rec2 come from the candidate kernel launched just before
+    const int64_t P = ws.P;
+    const int i = threadIdx.x & 15;
+    const int gb = (int)(threadIdx.x & 16u);
+    const int64_t p = blockIdx.x * (int64_t)16 + (threadIdx.x >> 4);
+    const bool live = p < P;
+    const int64_t pp = live ? p : P - 1;
+    const bool dot = i < n;
+    uint64_t idx;
+    if (closed_nb > 0) {  // closed walk: lexicographic minimum of the pixel's records (lane b holds record b)
+        double be = INFINITY;
+        idx = ~0ull;
+        if (i < closed_nb) {
+            const double2 r = ws.rec2[(int64_t)i * P + pp];
+            const uint64_t i2 = (uint64_t)(uint32_t)__double_as_longlong(r.y);
+            if (i2 != 0xffffffffull) {
+                be = r.x;
+                idx = i2;
+            }
+        }
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) {
+            const double e2 = __shfl_xor_sync(0xffffffffu, be, o);
+            const uint64_t i2 = __shfl_xor_sync(0xffffffffu, idx, o);
+            qa_lexmin(be, idx, e2, i2);
+        }
+    } else {
+        idx = ws.best[pp];
+    }
+    const bool empty = idx == ~0ull;
+    const uint64_t cnt = dot ? (uint64_t)ws.cnt[(int64_t)i * P + pp] : 1ull;
+    const int32_t base = dot ? ws.base[(int64_t)i * P + pp] : 0;
+    const double nc = dot ? ws.nc[(int64_t)i * P + pp] : 0.0;
+    // suffix products S_i = prod_{j > i} cnt_j: inclusive scan from the right, then one lane to the left
+    uint64_t incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        const uint64_t t = __shfl_down_sync(0xffffffffu, incl, o, 16);
+        if (i + o < 16) incl *= t;
+    }
+    uint64_t suf = __shfl_down_sync(0xffffffffu, incl, 1, 16);
+    if (i == 15) suf = 1ull;
+    const int32_t dg = empty ? 0 : (int32_t)((idx / suf) % cnt);
+    const int32_t Ni = empty ? -1 : base + dg;
+    const double d = dot ? (double)Ni - nc : 0.0;
+    double row = 0.0;
+    const int ii = dot ? i : 0;
+    for (int j = 0; j < n; ++j) row = fma(sM[ii * n + j], __shfl_sync(0xffffffffu, d, gb + j), row);
+    double E = dot ? d * row : 0.0;
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) E += __shfl_xor_sync(0xffffffffu, E, o);
+    if (live && dot) outN[p * n + i] = Ni;
+    if (live && i == 0) outE[p] = empty ? INFINITY : 0.5 * E;
+    if (closed_nb > 0 && stats) {  // C(n, k) states were scored, k = N_hat - sum base
+        int sb = base;
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) sb += __shfl_xor_sync(0xffffffffu, sb, o);
+        int64_t scored = 0;
+        const int k = N_hat - sb;
+        if (live && i == 0 && k >= 0 && k <= n) {
+            scored = 1;
+            for (int q = 1; q <= k; ++q) scored = scored * (n - k + q) / q;
+        }
+        qa_warp_count(&stats->n_candidates_scored, scored);
+    }
 }
 
 // FP64 issue-rate probe: 8 independent DFMA chains per thread.
@@ -585,8 +664,14 @@ cudaError_t qa_launch_enumerate(const QaDevModel *d_model, int n, QaWorkspace ws
 }
 
 cudaError_t qa_launch_finalize(const QaDevModel *d_model, const double *d_Vg, QaWorkspace ws, int32_t *d_N, double *d_E,
-                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream, int closed_nb, int N_hat)
+                               double *d_Vsensor, qa_stats *d_stats, cudaStream_t stream, int closed_nb, int N_hat, int n_lanes)
 {
+    if (n_lanes > 8) {  // 9..16 search dots, no sensor dots: sixteen lanes per pixel
+        qa_plan_add("qa_finalize_lanes_kernel");
+        const unsigned blocks = (unsigned)((ws.P + 15) / 16);
+        return qa_launch_pdl(qa_finalize_lanes_kernel, dim3(blocks), dim3(256), stream, d_model, ws, d_N, d_E, closed_nb, N_hat,
+                             d_stats);
+    }
     qa_plan_add("qa_finalize_kernel");
     const unsigned blocks = (unsigned)((ws.P + FIN_THREADS - 1) / FIN_THREADS);
     return qa_launch_pdl(qa_finalize_kernel, dim3(blocks), dim3(FIN_THREADS), stream, d_model, d_Vg, ws, d_N, d_E, d_Vsensor,
