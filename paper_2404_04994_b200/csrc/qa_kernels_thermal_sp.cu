@@ -13,8 +13,10 @@
 // minimum lies at most G = sum_{i<j} M_ij above ref_pix, so Z >= exp(-beta G): the launcher uses this kernel only while
 // beta G <= 600 (far from underflow; a factor that does underflow belongs to weights < e^-100 of the dominant one) and
 // for Maxwell models; everything else runs the two-pass Gray kernel of qa_kernels_thermal.cu.
-// E_min (optional output) is the exact minimum of A[u] + (B[w] + QL[u,w]) over the set (a min-plus pass, 1 DADD + 1 DSETP).
-// FP64-pipe instructions per candidate: 2 DFMA (+ 2 for E_min); per thread 8 exp + ~150 for the factors and marginals.
+// E_min (optional output): a lower bound per thread exactly as pass 1 of the min-plus walk forms it (1 DADD + 1/2 integer
+// min3 per candidate), then the threads within 2 units of the pixel's smallest bound (normally one) are re-scored exactly
+// by all threads of the pixel together.
+// FP64-pipe instructions per candidate: 2 DFMA (+ 1 DADD for E_min); per thread 8 exp + ~150 for the factors and marginals.
 // Deterministic: fixed shuffle / shared-memory reduction order.
 #include "qa_internal.cuh"
 
@@ -53,6 +55,9 @@ __global__ void __launch_bounds__(SP_THREADS, 2) qa_thermal_sp_kernel(const QaDe
     __shared__ double sIn[PPB][N + 1];
     __shared__ double sRed[NG][NR];
     __shared__ double sMin[NG];
+    __shared__ unsigned sLmin[NG];
+    __shared__ int sCnt[PPB];
+    __shared__ double sSurv[EMIN ? SP_THREADS : 1][NL + 1];  // survivors of the E_min bound: h'_0..7, be
 
     const unsigned t = threadIdx.x & (TPP - 1);
     const int slot = threadIdx.x >> NH;
@@ -92,26 +97,6 @@ __global__ void __launch_bounds__(SP_THREADS, 2) qa_thermal_sp_kernel(const QaDe
         double ref = be;
 #pragma unroll
         for (int j = 0; j < NL; ++j) ref += fmin(0.0, hp[j]);
-
-        // ---- E_min: exact minimum of A[u] + (B[w] + QL[u,w])
-        double emin = INFINITY;
-        if (EMIN) {
-            double B[16];
-            B[0] = 0.0;
-#pragma unroll
-            for (int w = 1; w < 16; ++w) B[w] = B[w & (w - 1)] + hp[sp_ctz(w)];
-#pragma unroll
-            for (int u = 0; u < 16; ++u) {
-                double m = B[0] + tab.QL[u << 4];
-#pragma unroll
-                for (int w = 1; w < 16; ++w) m = fmin(m, B[w] + tab.QL[(u << 4) | w]);
-                double a = be;
-#pragma unroll
-                for (int j = 3; j >= 0; --j)
-                    if ((u >> j) & 1) a += hp[4 + j];
-                emin = fmin(emin, a + m);
-            }
-        }
 
         // ---- weights: per-bit factors normalised to max 1
         double on[NL], off[NL];
@@ -176,16 +161,88 @@ __global__ void __launch_bounds__(SP_THREADS, 2) qa_thermal_sp_kernel(const QaDe
         for (int o = W / 2; o > 0; o >>= 1) {
 #pragma unroll
             for (int k = 0; k < NR; ++k) val[k] += __shfl_xor_sync(0xffffffffu, val[k], o);
-            if (EMIN) emin = fmin(emin, __shfl_xor_sync(0xffffffffu, emin, o));
         }
         if ((threadIdx.x & (W - 1)) == 0) {
 #pragma unroll
             for (int k = 0; k < NR; ++k) sRed[grp_id][k] = val[k];
-            sMin[grp_id] = emin;
         }
+        // ---- E_min, step 1: a lower bound of the thread's smallest energy as in pass 1 of the min-plus walk (positivity
+        // offsets from |h_j|, one DADD per candidate, integer minima on the high words: qa_kernels_minplus.cu); the threads
+        // within 2 of the pixel's smallest bound are re-scored exactly below
+        unsigned Lb = 0xffffffffu;
+        if (EMIN) {
+            double offw = EC, offu = 0.0;
+#pragma unroll
+            for (int j = 0; j < NL; ++j) {
+                if (j < 4)
+                    offw += fabs(sIn[slot][N - 1 - j]);
+                else
+                    offu += fabs(sIn[slot][N - 1 - j]);
+            }
+            double B[16];
+            B[0] = offw;
+#pragma unroll
+            for (int w = 1; w < 16; ++w) B[w] = B[w & (w - 1)] + hp[sp_ctz(w)];
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                unsigned m = 0xffffffffu;
+#pragma unroll
+                for (int w = 0; w < 16; w += 2)
+                    m = min(m, min((unsigned)__double2hiint(B[w] + tab.QL[(u << 4) | w]),
+                                   (unsigned)__double2hiint(B[w + 1] + tab.QL[(u << 4) | (w + 1)])));
+                double a = be + offu;
+#pragma unroll
+                for (int j = 3; j >= 0; --j)
+                    if ((u >> j) & 1) a += hp[4 + j];
+                Lb = min(Lb, (unsigned)__double2hiint(a + __hiloint2double((int)m, 0)));
+            }
+        }
+
+        unsigned Lg = Lb;
+        if (EMIN) {
+#pragma unroll
+            for (int o = W / 2; o > 0; o >>= 1) Lg = min(Lg, __shfl_xor_sync(0xffffffffu, Lg, o));
+        }
+        if ((threadIdx.x & (W - 1)) == 0) sLmin[grp_id] = Lg;
+        if (EMIN && threadIdx.x < PPB) sCnt[threadIdx.x] = 0;
         __syncthreads();
         const int64_t p = p0 + slot;
         const int g0 = slot * GPP;
+        if (EMIN) {
+            // ---- E_min, step 2: the survivors publish (h'_0..7, be); every thread of the pixel then scores its share of a
+            // survivor's 2^8 candidates from the definition of the split, e = be + sum_{j in c} h'_j + QL[c]
+            unsigned Lp = 0xffffffffu;
+#pragma unroll
+            for (int gq = 0; gq < GPP; ++gq) Lp = min(Lp, sLmin[g0 + gq]);
+            if (Lb <= Lp + 2u) {
+                const int pos = atomicAdd(&sCnt[slot], 1);
+                double *dst = sSurv[slot * TPP + pos];
+#pragma unroll
+                for (int j = 0; j < NL; ++j) dst[j] = sIn[slot][N - 1 - j] + v[j];
+                double be2 = sIn[slot][N] + QH;
+#pragma unroll
+                for (int jh = 0; jh < NH; ++jh)
+                    if ((t >> jh) & 1u) be2 += sIn[slot][N - 1 - NL - jh];
+                dst[NL] = be2;
+            }
+            __syncthreads();
+            double em = INFINITY;
+            const int ns = sCnt[slot];
+            for (int sv = 0; sv < ns; ++sv) {
+                const double *src = sSurv[slot * TPP + sv];
+                for (int c = (int)t; c < 256; c += TPP) {
+                    double e = src[NL];
+#pragma unroll
+                    for (int j = NL - 1; j >= 0; --j)
+                        if ((c >> j) & 1) e += src[j];
+                    em = fmin(em, e + tab.QL[c]);
+                }
+            }
+#pragma unroll
+            for (int o = W / 2; o > 0; o >>= 1) em = fmin(em, __shfl_xor_sync(0xffffffffu, em, o));
+            if ((threadIdx.x & (W - 1)) == 0) sMin[grp_id] = em;
+            __syncthreads();
+        }
         for (int q = (int)t; q <= N && p < P; q += TPP) {  // output q < N: dot q; q = N: E_min
             if (q < N) {
                 double Z = 0.0;
