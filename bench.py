@@ -2,7 +2,12 @@
 """bench.py -- throughput of the ground-state charge search on the headline workload (BASELINE.json configs[3]:
 open 4x4 grid of 16 dots, default algorithm, 100x100 pixels, 2^16 candidates per pixel, fp64).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4|config5|small|thermal]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload config4|config5|small|thermal|closed16|sweep] [--no-parity] [--no-secondary]
+
+The default run (config4) prints ONE JSON line: the headline, its roofline, the oracle baseline, the end-to-end number, the
+opt-in walk variants, the full-size parity report of all five BASELINE.json configs ("parity") and the other workloads
+("secondary": config5, small, closed16, thermal, sweep).  --workload X prints the line of that workload alone.
 
 One "step" = one pass of the whole hot path (prologue -> candidate walk -> finalize) over
 one 100x100 diagram.  Prints ONE JSON line (rank 0).  Multi-GPU: one process per GPU (torchrun), every rank runs its own

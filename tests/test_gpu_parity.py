@@ -268,6 +268,21 @@ def test_closed_default_large_arrays(api, n):
     assert g["plan"][0][1] == "qa_closed_walk_kernel"
 
 
+def test_closed16_full_size_every_pixel(api):
+    """bench.py's closed16 workload in its launch configuration: the config-4 model and sweep as a CLOSED array with N_hat = 16
+    (PAPER.md L496), all 10^4 pixels against the oracle (OpenMP), counters included."""
+    w = wl.config4(100, 100)
+    w.regime, w.N_hat = "closed", 16
+    g = run_gpu(api, w)
+    om = oracle.Model(w.C_dd, w.C_gd)
+    o = om.ground_state(w.Vg, regime="closed", N_hat=16, n_threads=os.cpu_count() or 1)
+    rep = compare(g["N"], g["E"], o, om.EC, gpu_x=g["xcont"])
+    assert rep["unexcused"] == 0 and rep["qp_pixels"] > 5000
+    assert g["plan"][0] == ["qa_prologue_kernel", "qa_closed_walk_kernel", "qa_finalize_lanes_kernel"]
+    assert g["stats"]["n_candidates_scored"] == int(o["n_scored"].sum()) and g["stats"]["n_qp_failed"] == 0
+    assert (g["N"].sum(1) == 16).all()
+
+
 def test_closed_default_edge_totals(api):
     """N_hat = 0 (only the all-zero state), N_hat far above what the gates ask for, and P not a multiple of the pixels per
     CTA, on a 10-dot and a 16-dot array."""
