@@ -279,6 +279,12 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
             return QA_OK;
         }
     }
+    // open default search of 9..12 dots without sensor dots: the whole path in one kernel, a warp per two pixels
+    if (!closed && alg == QA_ALG_DEFAULT && n > QA_FUSED_MAXN && n <= 12 && m->ns == 0 && variant != 0) {
+        QA_CUDA(qa_launch_fused_mid(m->dev, n, m->walk, d_Vg, P, a, d_N, d_E, d_xcont, d_stats, stream));
+        timing_mark(stream);
+        return QA_OK;
+    }
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, d_xcont, d_stats, stream, variant != 0));
     timing_mark(stream);
     // the min-plus walk needs M >= 0 entrywise (its positivity offsets), which holds for a Maxwell c_dd

@@ -223,11 +223,34 @@ def test_config5_open_grid8_default_and_thresholded(api):
 def test_all_sizes_default_open(api, n):
     w = wl.random_open(n, n + (n % 3), 301 if n <= 10 else (67 if n <= 13 else 37), seed=50 + n)
     rep, g, o = check(api, w, algorithm="default")
-    if n <= 8:   # the one-kernel path above; the three-kernel path (static walk) below
-        assert g["plan"][0] == ["qa_fused_open_kernel"]
+    if n <= 12:   # the one-kernel paths above; the three-kernel path (static walk) below
+        assert g["plan"][0] == (["qa_fused_open_kernel"] if n <= 8 else ["qa_fused_mid_kernel"])
         rep, g0, o = check(api, w, variant=0, algorithm="default")
         assert g0["plan"][0] == ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"]
         assert np.array_equal(g["N"], g0["N"])
+
+
+@pytest.mark.parametrize("n,g,P", [(9, 9, 1003), (10, 13, 517), (11, 11, 259), (12, 12, 130), (12, 64, 33), (9, 2, 17)])
+def test_fused_mid_kernel(api, n, g, P):
+    """Open default search of 9..12 dots in one kernel (a warp per two pixels): sizes that are not multiples of the 16 pixels
+    of a CTA (a ragged last CTA, an odd last pixel of a warp), more gates than dots up to the 64-gate limit and fewer, QP
+    pixels with one to three and with more clamped dots (the serial solver), a general SPD c_dd, extreme gate voltages;
+    element by element against the oracle, counters included, and bit-identical N to the three-kernel path."""
+    w = wl.random_open(n, g, P, seed=820 + n + g, lo=-0.9, hi=3.1)
+    rep, gg, o = check(api, w, algorithm="default")
+    assert gg["plan"][0] == ["qa_fused_mid_kernel"] and gg["stats"]["n_qp_pixels"] > 0
+    assert gg["stats"]["n_candidates_scored"] == P * 2 ** n
+    rep0, g0, _ = check(api, w, variant=0, algorithm="default")
+    assert np.array_equal(gg["N"], g0["N"])
+    if g == n:
+        wg = wl.random_general(n, n, 77, seed=860 + n)
+        rep, gg, o = check(api, wg, algorithm="default")
+        assert gg["plan"][0] == ["qa_fused_mid_kernel"] and gg["stats"]["n_qp_pixels"] > 0
+        rng = np.random.default_rng(n)
+        w.Vg = np.ascontiguousarray(np.concatenate([w.Vg[:20], -40.0 * np.abs(rng.standard_normal((9, g))), w.Vg[:5] * 30.0,
+                                                    np.zeros((2, g))]))
+        w.W, w.H = w.Vg.shape[0], 1
+        check(api, w, algorithm="default")
 
 
 @pytest.mark.parametrize("n", [1, 2, 3, 6, 9, 11])
