@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(FM_THREADS) qa_fused_mid_kernel(const QaDevMod
 {
     constexpr int NH = 5, NL = N - NH;
     static_assert(N >= 9 && N <= 12, "five high bits = one lane each, 4..7 low bits per lane");
-    __shared__ double sCgT[QA_MAXG * N], sC[N * N], sMT[N * N], sV[FM_PPB][QA_MAXG], sX[FM_PPB][N];
+    __shared__ double sCgT[QA_MAXG * N], sC[N * N], sMT[N * N], sV[FM_PPB][QA_MAXG], sX[FM_PPB][2 * N], sC1[N];
     const int g = mdl->g;
     const int tid = threadIdx.x;
     for (int e = tid; e < N * N; e += FM_THREADS) {
@@ -49,6 +49,7 @@ __global__ void __launch_bounds__(FM_THREADS) qa_fused_mid_kernel(const QaDevMod
         sC[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
     }
     for (int e = tid; e < N * g; e += FM_THREADS) sCgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
+    if (tid < N) sC1[tid] = mdl->C1[tid];
     const int64_t p0 = (int64_t)blockIdx.x * FM_PPB;
     for (int e = tid; e < FM_PPB * g; e += FM_THREADS) {
         const int64_t pe = p0 + e / g;
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(FM_THREADS) qa_fused_mid_kernel(const QaDevMod
 
     // ---- S1-S4 + base-point gradient, sixteen lanes per pixel
     QaLaneOut lo;
-    qa_lanes_pixel<N>(sCgT, sC, sMT, sV[s], sX[s], g, i, gb, dot, args, lo);
+    qa_lanes_pixel<N>(sCgT, sC, sMT, sC1, 1.0, sV[s], sX[s], g, i, gb, dot, args, lo);  // (open: 1^T C 1 is not read)
     const double h = dot ? lo.gi + 0.5 * sMT[i * N + i] : 0.0;  // E(base + e_i) - E(base)
 
     // ---- S5-S6: the warp's two pixels, one after the other

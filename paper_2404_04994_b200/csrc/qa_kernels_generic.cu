@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(PRO_THREADS) qa_prologue_kernel(const QaDevMod
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Prologue of OPEN arrays with 9..16 dots, sixteen lanes per pixel (lane i <-> dot i).  The thread-per-pixel kernel above
+// Prologue of arrays with 9..16 dots (open and closed), sixteen lanes per pixel (lane i <-> dot i).  The thread-per-pixel kernel above
 // puts 10^4 pixels on 79 CTAs -- two warps per SM, each thread a chain of ~600 dependent FP64 instructions.  Here a pixel's
 // N_c,i (the same fma chain over k as everywhere: reading R1), the candidate range of dot i and the row i of M d0 belong
 // to lane i, the other dots' values travel by shuffles, and the outputs go through shared memory so that the stores to
@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel
     constexpr int LPP = 16, PPB = 256 / LPP;
     static_assert(N > 8 && N <= LPP, "sixteen lanes per pixel");
     __shared__ double sCgT[QA_MAXG * N], sC[N * N], sMT[N * N], sV[PPB][QA_MAXG];
-    __shared__ double sH[N][PPB], sNc[N][PPB], sX[PPB][N];
+    __shared__ double sH[N][PPB], sNc[N][PPB], sX[PPB][2 * N], sC1[N];
     __shared__ int32_t sBase[N][PPB], sCnt[N][PPB];
     const int g = mdl->g;
     const int tid = threadIdx.x;
@@ -112,6 +112,8 @@ __global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel
         sC[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
     }
     for (int e = tid; e < N * g; e += 256) sCgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
+    if (tid < N) sC1[tid] = mdl->C1[tid];
+    const double oneC1 = mdl->oneC1;
     const int64_t P = ws.P;
     const int64_t p0 = (int64_t)blockIdx.x * PPB;
     for (int e = tid; e < PPB * g; e += 256) {
@@ -131,7 +133,7 @@ __global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel
     const bool dot = i < N;
 
     QaLaneOut lo;
-    qa_lanes_pixel<N>(sCgT, sC, sMT, sV[s], sX[s], g, i, gb, dot, args, lo);
+    qa_lanes_pixel<N>(sCgT, sC, sMT, sC1, oneC1, sV[s], sX[s], g, i, gb, dot, args, lo);
     const double nc = lo.nc, x = lo.x, gi = lo.gi, e0 = lo.e0;
     const int32_t base = lo.base, cnt = lo.cnt;
     const uint64_t total = lo.total;
@@ -165,8 +167,9 @@ __global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel
         qa_warp_count(&stats->n_qp_pixels, (one && neg0 != 0u) ? 1 : 0);
         qa_warp_count(&stats->n_qp_rounds, one ? rounds : 0);
         qa_warp_count(&stats->n_qp_failed, (one && failed) ? 1 : 0);
+        qa_warp_count(&stats->n_threshold_doublings, one ? lo.doublings : 0);
         qa_warp_count(&stats->n_candidates_enumerated, one ? (int64_t)total : 0);
-        qa_warp_count(&stats->n_candidates_scored, one ? (int64_t)total : 0);  // open: all are scored
+        qa_warp_count(&stats->n_candidates_scored, (one && !args.closed) ? (int64_t)total : 0);  // open: all are scored
     }
 }
 
@@ -524,7 +527,10 @@ cudaError_t qa_launch_prologue(const QaDevModel *d_model, int n, int g, const do
                                QaCallArgs args, double *d_xcont, qa_stats *d_stats, cudaStream_t stream, bool lanes)
 {
     (void)g;
-    if (lanes && !args.closed && n > 8) {  // open arrays of 9..16 dots: sixteen lanes per pixel
+    // 9..16 dots: sixteen lanes per pixel.  Closed arrays clamp many dots per pixel; there the lane-parallel QP (conjugate
+    // gradients, ~16x the warp instructions of the serial solver but 16x the warps) wins only for 12..15 dots (measured:
+    // bench.py --workload sweep), so the other closed sizes keep the thread-per-pixel kernel
+    if (lanes && n > 8 && (!args.closed || (n >= 12 && n <= 15))) {
         qa_plan_add("qa_prologue_lanes_kernel");
 #define CALL(NN) launch_prologue_lanes_n<NN>(d_model, d_Vg, ws, args, d_xcont, d_stats, stream)
         switch (n) {
