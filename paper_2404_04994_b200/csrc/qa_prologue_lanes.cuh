@@ -111,9 +111,11 @@ __device__ __forceinline__ void qa_lanes_pixel(const double *__restrict__ sCgT, 
             if (!__any_sync(0xffffffffu, work)) break;
             const unsigned Aw = work ? A : 1u;
             const bool inA = dot && ((Aw >> i) & 1u);
+            // (which of the two solvers a pixel gets depends on that pixel alone, not on the other pixel of its warp)
             const bool small = !closed && __popc(Aw) <= 3;
-            if (__all_sync(0xffffffffu, small || !work)) {
-                // open, |A| <= 3 in every working pixel of the warp: explicit inverse (qa_qp_small_open's arithmetic)
+            const bool workS = work && small, workC = work && !small;
+            if (__any_sync(0xffffffffu, workS)) {
+                // open, |A| <= 3: explicit inverse (qa_qp_small_open's arithmetic)
                 const int ia = __ffs(Aw) - 1;
                 const unsigned A2 = Aw & (Aw - 1);
                 const int ib = A2 ? __ffs(A2) - 1 : ia;
@@ -121,7 +123,7 @@ __device__ __forceinline__ void qa_lanes_pixel(const double *__restrict__ sCgT, 
                 const int ic = A3 ? __ffs(A3) - 1 : ib;
                 const double ca = __shfl_sync(0xffffffffu, nc, gb + ia), cb = __shfl_sync(0xffffffffu, nc, gb + ib),
                              cc = __shfl_sync(0xffffffffu, nc, gb + ic);
-                if (work) {
+                if (workS) {
                     double ya, yb = 0.0, yc = 0.0;
                     if (A3) {
                         const double a = sC[ia * N + ia], b = sC[ia * N + ib], cq = sC[ia * N + ic];
@@ -146,8 +148,8 @@ __device__ __forceinline__ void qa_lanes_pixel(const double *__restrict__ sCgT, 
                     x = ((A >> i) & 1u) ? 0.0 : sx;  // clamped components are exactly 0 (R3)
                     if (ya < -1e-9 * scale || yb < -1e-9 * scale || yc < -1e-9 * scale) failed = true;  // KKT
                 }
-                continue;
             }
+            if (!__any_sync(0xffffffffu, workC)) continue;
             // ---- conjugate gradients on C_AA a = -c_A and (closed) C_AA b = C_AF 1_F; lane a <-> unknown a
             double rF = 0.0;  // sum_{f in F} C[i][f]
             if (closed) {
@@ -156,11 +158,12 @@ __device__ __forceinline__ void qa_lanes_pixel(const double *__restrict__ sCgT, 
                     if (!((Aw >> j) & 1u)) rF += sC[ii * N + j];
             }
             double za = 0.0, zb = 0.0;
-            double ra = (work && inA) ? -nc : 0.0, rb = (work && inA && closed) ? rF : 0.0;
+            double ra = (workC && inA) ? -nc : 0.0, rb = (workC && inA && closed) ? rF : 0.0;
             double pa = ra, pb = rb;
             double rsa = qa_gsum(ra * ra), rsb = closed ? qa_gsum(rb * rb) : 0.0;
             const double tola = 1e-32 * rsa, tolb = 1e-32 * rsb;
-            const int itmax = __reduce_max_sync(0xffffffffu, work ? __popc(Aw) + 2 : 0);
+            const int myit = workC ? __popc(Aw) + 2 : 0;  // a pixel's own iteration count (not its warp neighbour's)
+            const int itmax = __reduce_max_sync(0xffffffffu, myit);
             for (int it = 0; it < itmax; ++it) {
                 __syncwarp();
                 if (dot) {
@@ -177,20 +180,20 @@ __device__ __forceinline__ void qa_lanes_pixel(const double *__restrict__ sCgT, 
                 }
                 if (!inA) Apa = Apb = 0.0;
                 const double da = qa_gsum(pa * Apa);
-                const double ala = (rsa > tola && da > 0.0) ? rsa / da : 0.0;
+                const double ala = (it < myit && rsa > tola && da > 0.0) ? rsa / da : 0.0;
                 za = fma(ala, pa, za);
                 ra = fma(-ala, Apa, ra);
                 const double rsa2 = qa_gsum(ra * ra);
-                const double bea = (rsa > tola && rsa > 0.0) ? rsa2 / rsa : 0.0;
+                const double bea = (it < myit && rsa > tola && rsa > 0.0) ? rsa2 / rsa : 0.0;
                 pa = fma(bea, pa, ra);
                 rsa = rsa2;
                 if (closed) {
                     const double db = qa_gsum(pb * Apb);
-                    const double alb = (rsb > tolb && db > 0.0) ? rsb / db : 0.0;
+                    const double alb = (it < myit && rsb > tolb && db > 0.0) ? rsb / db : 0.0;
                     zb = fma(alb, pb, zb);
                     rb = fma(-alb, Apb, rb);
                     const double rsb2 = qa_gsum(rb * rb);
-                    const double beb = (rsb > tolb && rsb > 0.0) ? rsb2 / rsb : 0.0;
+                    const double beb = (it < myit && rsb > tolb && rsb > 0.0) ? rsb2 / rsb : 0.0;
                     pb = fma(beb, pb, rb);
                     rsb = rsb2;
                 }
@@ -216,7 +219,7 @@ __device__ __forceinline__ void qa_lanes_pixel(const double *__restrict__ sCgT, 
                 const double s2 = qa_gsum(fr ? rF : 0.0), s3 = qa_gsum(fr ? Cb : 0.0);
                 lam = ((Nhat - s0) - s1) / (s2 - s3);
             }
-            if (work) {
+            if (workC) {
                 const double yi = za - lam * zb;  // multiplier direction of a clamped lane
                 double sx = nc + Ca;
                 if (closed) sx += lam * (rF - Cb);
