@@ -533,6 +533,35 @@ def test_deterministic_across_runs_and_streams(api):
 
 
 # ---- exact ties (reading R6): the lexicographically smallest N among bitwise-equal energies ------------------------
+@pytest.mark.parametrize("n,regime", [(5, "open"), (8, "open"), (10, "open"), (13, "open"), (16, "open"), (13, "closed"), (16, "closed")])
+def test_pixels_are_independent_of_their_neighbours(api, n, regime):
+    """Pixel-range sharding relies on it: the result of a pixel must not depend on which pixels share its
+    thread, warp, CTA or call.  The same gate vectors in a shuffled order, and a sub-range of them, must give bit-identical
+    N, E and x (two pixels per thread / warp, the CTA bucket sort, pixel pairs of the min-plus walk, the per-pixel choice of
+    the QP solver in the sixteen-lanes prologue)."""
+    w = wl.random_open(n, n, 419, seed=930 + n, lo=-0.8, hi=3.0)
+    w.regime, w.N_hat = regime, n
+    ref = run_gpu(api, w)
+    perm = np.random.default_rng(n).permutation(w.P)
+    w2 = wl.random_open(n, n, 419, seed=930 + n, lo=-0.8, hi=3.0)
+    w2.regime, w2.N_hat = regime, n
+    w2.Vg = np.ascontiguousarray(w.Vg[perm])
+    g2 = run_gpu(api, w2)
+    for key in ("N", "E", "xcont"):
+        assert np.array_equal(ref[key][perm], g2[key]), key
+    w3 = wl.random_open(n, n, 419, seed=930 + n, lo=-0.8, hi=3.0)
+    w3.regime, w3.N_hat = regime, n
+    w3.Vg = np.ascontiguousarray(w.Vg[37:230])
+    w3.W = 193
+    g3 = run_gpu(api, w3)
+    for key in ("N", "E", "xcont"):
+        assert np.array_equal(ref[key][37:230], g3[key]), key
+    for algkw in (dict(algorithm="thresholded", t=0.4),):
+        a = run_gpu(api, w, **algkw)
+        b = run_gpu(api, w2, **algkw)
+        assert np.array_equal(a["N"][perm], b["N"]) and np.array_equal(a["E"][perm], b["E"])
+
+
 @pytest.mark.parametrize("n", [2, 5, 8, 10, 12, 13, 16])
 def test_exact_ties_fall_to_the_lexicographically_smallest_state(api, n):
     """Diagonal c_dd with entries in {1/4, 1, 4} (so M = c_dd^-1 is exact), C_gd = I and N_c on quarter-integers: every
