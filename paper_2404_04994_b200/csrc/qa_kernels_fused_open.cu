@@ -7,10 +7,11 @@
 // floor is HBM (104 B per pixel at n = g = 8); the arithmetic next to it is ~200 FP64 instructions of per-pixel prologue
 // and epilogue (N_c: n g FMA, M d0: n^2 FMA, E(N*) from the definition: n^2 + n FMA) plus the candidate walk.  Every FMA
 // of the prologue takes one operand from a per-MODEL matrix, i.e. a warp-uniform value that has to come out of shared
-// memory (the model differs per CTA, so the constant bank is not available): a broadcast LDS.128 returns 512 B for two
-// operands, four SM cycles of the shared-memory pipe, while the FP64 pipe needs 2 cycles per scheduler for the two FMAs
-// -- with one pixel per thread the kernel would be bound by shared-memory return bandwidth at 1/4 of the FP64 rate.  Hence
-// TWO pixels per thread everywhere (prologue, walk, epilogue): every uniform operand fetched serves two FMAs / DADDs.
+// memory (the model differs per CTA, so the constant bank is not available).  The kernel is a template over PX = pixels
+// per thread.  PX = 2 halves that operand traffic (every uniform operand serves two FMAs / DADDs) but needs 128 registers
+// and 48 KB of shared memory per CTA (N_c and the base point parked there), i.e. 16 warps per SM; measured, the kernels
+// then run at 20-45 % of the FP64 pipe with 37-60 % of the issue slots: bound by latency, not by operand bandwidth.
+// PX = 1 (64 registers, 20-28 KB, 32 warps per SM) is what the launcher instantiates: config 5 1.49 -> 1.21 ms per step.
 //
 // Register discipline: nothing in the common path is dynamically indexed, so nothing lives in local memory.  The QP
 // (L106, reading R3) is solved in closed form in registers for one to three clamped dots (all but 3 in 10^5 pixels of the
@@ -18,11 +19,11 @@
 // with the general solver (fo_slow_pixel), whose work arrays never touch the frame of the common path.
 //
 // Candidate walk.
-//   default:      the static counting-order walk of qa_kernels_walk.cu over all 2^n patterns, two pixels at once (3 FP64
-//                 instructions per candidate and pixel, one table entry per candidate for both pixels).
+//   default:      the static counting-order walk of qa_kernels_walk.cu over all 2^n patterns, the thread's PX pixels at once
+//                 (3 FP64 instructions per candidate and pixel, one table entry per candidate for all of them).
 //   thresholded:  the number of free dots k differs from pixel to pixel (2^k candidates: 4.3 on average at t = 0.2, 25.6
 //                 at t = 0.5, but up to 256), so a warp of neighbouring pixels would run at the pace of its largest set.  The
-//                 256 pixels of a CTA are therefore bucket-sorted by k in shared memory and every thread walks two
+//                 pixels of a CTA are therefore bucket-sorted by k in shared memory and every thread walks PX
 //                 pixels of (nearly) equal k.  The walk is the counting-order walk restricted to the free dots: with the
 //                 free dots f_0 < f_1 < .. (bit positions) the step st-1 -> st sets free bit j = ctz(st) and clears the
 //                 free bits below it, so the linear part moves by c_j = h_{f_j} - sum_{i<j} h_{f_i} (stored per pixel in
@@ -35,8 +36,9 @@
 namespace {
 
 constexpr int FO_THREADS = 128;
-constexpr int FO_PX = 2;                        // pixels per thread
-constexpr int FO_PIX = FO_THREADS * FO_PX;      // pixels per CTA
+constexpr int FO_PX_RUN = 1;  // pixels per thread the launcher instantiates (measured, config 5: 1.21 ms per step vs 1.49 with 2)
+// PX = pixels per thread (2: every uniform operand serves two FMAs; 1: half the registers and shared memory per CTA, twice
+// the CTAs per SM -- the thresholded kernels are bound by latency, not by the FP64 pipe), PIX = FO_THREADS * PX per CTA
 
 __host__ __device__ constexpr int fo_ctz(int k)
 {
@@ -89,26 +91,26 @@ __device__ __forceinline__ int fo_qp_open(const double *__restrict__ sC, const d
     return rounds;
 }
 
-template <int N, bool THR>
+template <int N, bool THR, int PIX>
 struct FoSort {  // thresholded: bookkeeping of the bucket sort and the walk
-    unsigned long long xm[THR ? FO_PIX : 1];  // XOR masks of the steps, 8 bits per free dot
-    unsigned short order[THR ? FO_PIX : 1];   // pixel slots sorted by the number of free dots, descending
-    unsigned char kfree[THR ? FO_PIX : 1];    // number of free dots
-    unsigned char wkey[THR ? FO_PIX : 1];     // winning pattern
+    unsigned long long xm[THR ? PIX : 1];  // XOR masks of the steps, 8 bits per free dot
+    unsigned short order[THR ? PIX : 1];   // pixel slots sorted by the number of free dots, descending
+    unsigned char kfree[THR ? PIX : 1];    // number of free dots
+    unsigned char wkey[THR ? PIX : 1];     // winning pattern
     int bucket[16];
 };
 
-template <int N, bool THR>
+template <int N, bool THR, int PIX>
 struct FoSmem {
     double MT[N * N];          // MT[j*N + i] = M[i][j]: the N values a column step needs are contiguous
     double C[N * N];           // c_dd, row-major (QP)
     double T[1 << N];          // pair table of the bit patterns: T[b] = QL[b] (bit j <-> dot N-1-j)
-    double nc[N][FO_PIX];      // N_c of every pixel slot, parked during the walk (registers: 4 CTAs per SM)
-    int32_t base[N][FO_PIX];   // ... and the base point
-    double cs[THR ? N : 1][FO_PIX];     // thresholded: c_j of the compacted free dots, per pixel slot
+    double nc[N][PIX];      // N_c of every pixel slot, parked during the walk (registers: 4 CTAs per SM)
+    int32_t base[N][PIX];   // ... and the base point
+    double cs[THR ? N : 1][PIX];     // thresholded: c_j of the compacted free dots, per pixel slot
     union {                    // C_gd is dead after S1 (a barrier separates it from the sort's first write)
         double CgT[QA_MAXG * N];   // CgT[k*N + i] = C_gd[i][k]
-        FoSort<N, THR> sort;
+        FoSort<N, THR, PIX> sort;
     };
 };
 
@@ -210,14 +212,15 @@ __device__ __forceinline__ int fo_bucket_rank(int *bucket, int key)
     return start + __popc(peers & ((1u << lane) - 1u));
 }
 
-template <int N, bool THR>
-__global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDevModel *const *__restrict__ models,
+template <int N, bool THR, int PX>
+__global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel(const QaDevModel *const *__restrict__ models,
                                                                    const double *__restrict__ Vg, int64_t P, int g,
                                                                    QaCallArgs args, int32_t *__restrict__ outN,
                                                                    double *__restrict__ outE, double *__restrict__ xcont,
                                                                    double *__restrict__ outVs, qa_stats *stats)
 {
-    __shared__ __align__(16) FoSmem<N, THR> sm;
+    constexpr int FO_PX = PX, FO_PIX = FO_THREADS * PX;
+    __shared__ __align__(16) FoSmem<N, THR, FO_PIX> sm;
     const int tid = threadIdx.x;
     // The thread's two pixels: slot = tid + px * FO_THREADS (coalescing: consecutive threads, consecutive rows).  The first
     // eight gate voltages of both rows are requested before anything else: their HBM round trip overlaps the staging of the
@@ -230,29 +233,28 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
         live[px] = p < P;
         gp[px] = (int64_t)blockIdx.y * P + (live[px] ? p : P - 1);
     }
-    const double *v0 = Vg + gp[0] * g, *v1 = Vg + gp[1] * g;
+    const double *vp[FO_PX];
+#pragma unroll
+    for (int px = 0; px < FO_PX; ++px) vp[px] = Vg + gp[px] * g;
     const bool vec = (g & 1) == 0 && (reinterpret_cast<uintptr_t>(Vg) & 15u) == 0;
-    auto load_chunk = [&](int k0, double (&a)[8], double (&b)[8]) {
-        if (vec) {
+    auto load_chunk = [&](int k0, double (&a)[FO_PX][8]) {
 #pragma unroll
-            for (int k = 0; k < 8; k += 2) {
-                double2 ta = make_double2(0.0, 0.0), tb = ta;
-                if (k0 + k < g) {
-                    ta = __ldg(reinterpret_cast<const double2 *>(v0 + k0 + k));
-                    tb = __ldg(reinterpret_cast<const double2 *>(v1 + k0 + k));
+        for (int px = 0; px < FO_PX; ++px) {
+            if (vec) {
+#pragma unroll
+                for (int k = 0; k < 8; k += 2) {
+                    double2 ta = make_double2(0.0, 0.0);
+                    if (k0 + k < g) ta = __ldg(reinterpret_cast<const double2 *>(vp[px] + k0 + k));
+                    a[px][k] = ta.x, a[px][k + 1] = ta.y;
                 }
-                a[k] = ta.x, a[k + 1] = ta.y, b[k] = tb.x, b[k + 1] = tb.y;
-            }
-        } else {
+            } else {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                a[k] = k0 + k < g ? __ldg(v0 + k0 + k) : 0.0;
-                b[k] = k0 + k < g ? __ldg(v1 + k0 + k) : 0.0;
+                for (int k = 0; k < 8; ++k) a[px][k] = k0 + k < g ? __ldg(vp[px] + k0 + k) : 0.0;
             }
         }
     };
-    double va[8], vb[8];
-    load_chunk(0, va, vb);
+    double va[FO_PX][8];
+    load_chunk(0, va);
     const QaDevModel *__restrict__ mdl = models[blockIdx.y];
     for (int e = tid; e < N * N; e += FO_THREADS) {
         sm.MT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
@@ -274,15 +276,15 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
         for (int i = 0; i < N; ++i) nc[px][i] = 0.0;
     // S1: N_c,i = fma(C_gd[i,k], V[k], acc), k ascending (R1), in chunks of 8 gates (all loads of a chunk before its FMAs)
     for (int k0 = 0; k0 < g; k0 += 8) {
-        if (k0 > 0) load_chunk(k0, va, vb);
+        if (k0 > 0) load_chunk(k0, va);
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
             if (k0 + k < g) {
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
                     const double cg = sm.CgT[(k0 + k) * N + i];
-                    nc[0][i] = fma(cg, va[k], nc[0][i]);
-                    nc[1][i] = fma(cg, vb[k], nc[1][i]);
+#pragma unroll
+                    for (int px = 0; px < FO_PX; ++px) nc[px][i] = fma(cg, va[px][k], nc[px][i]);
                 }
             }
         }
@@ -333,15 +335,15 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
 #pragma unroll
             for (int i = 0; i < N; ++i) {
                 const double mij = sm.MT[j * N + i];
-                grad[0][i] = fma(mij, d0[0][j], grad[0][i]);
-                grad[1][i] = fma(mij, d0[1][j], grad[1][i]);
+#pragma unroll
+                for (int px = 0; px < FO_PX; ++px) grad[px][i] = fma(mij, d0[px][j], grad[px][i]);
             }
         }
 #pragma unroll
         for (int b = 0; b < N; ++b) {
             const double hm = 0.5 * sm.MT[(N - 1 - b) * N + (N - 1 - b)];
-            hp[0][b] = grad[0][N - 1 - b] + hm;
-            hp[1][b] = grad[1][N - 1 - b] + hm;
+#pragma unroll
+            for (int px = 0; px < FO_PX; ++px) hp[px][b] = grad[px][N - 1 - b] + hm;
         }
     }
 
@@ -446,7 +448,7 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
         __syncthreads();
         // thread tid walks the pixels of rank tid (large sets first) and FO_PIX-1-tid (small sets): balanced pairs
 #pragma unroll 1
-        for (int half = 0; half < 2; ++half) {
+        for (int half = 0; half < FO_PX; ++half) {
             const int slot = sm.sort.order[half == 0 ? tid : FO_PIX - 1 - tid];
             const unsigned nst = 1u << sm.sort.kfree[slot];
             const unsigned long long xm = sm.sort.xm[slot];
@@ -491,8 +493,8 @@ __global__ void __launch_bounds__(FO_THREADS, 4) qa_fused_open_kernel(const QaDe
 #pragma unroll
         for (int i = 0; i < N; ++i) {
             const double mij = sm.MT[j * N + i];
-            row[0][i] = fma(mij, d[0][j], row[0][i]);
-            row[1][i] = fma(mij, d[1][j], row[1][i]);
+#pragma unroll
+            for (int px = 0; px < FO_PX; ++px) row[px][i] = fma(mij, d[px][j], row[px][i]);
         }
     }
 #pragma unroll
@@ -561,11 +563,13 @@ cudaError_t launch_fused_open_n(const QaDevModel *const *d_models, int n_models,
                                 QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
                                 qa_stats *d_stats, cudaStream_t stream)
 {
-    const dim3 grid((unsigned)((P + FO_PIX - 1) / FO_PIX), (unsigned)n_models);
+    const dim3 grid((unsigned)((P + FO_THREADS * FO_PX_RUN - 1) / (FO_THREADS * FO_PX_RUN)), (unsigned)n_models);
     if (args.alg == QA_ALG_DEFAULT)
-        qa_fused_open_kernel<N, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont, d_Vs, d_stats);
+        qa_fused_open_kernel<N, false, FO_PX_RUN><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont,
+                                                                                d_Vs, d_stats);
     else
-        qa_fused_open_kernel<N, true><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont, d_Vs, d_stats);
+        qa_fused_open_kernel<N, true, FO_PX_RUN><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont,
+                                                                               d_Vs, d_stats);
     return cudaGetLastError();
 }
 
