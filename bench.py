@@ -314,10 +314,20 @@ def run_ours(args, rank, world, local_rank):
                "d2h_bytes_per_step": int(sum(o["N"].numel() * 4 + o["E"].numel() * 8 for o in ho)),
                "api": "qa_ground_state_host (pinned host buffers)", "n_gpus_measured": 1}
 
-    cpu = None if args.no_cpu_baseline else cpu_baseline(args)
+    cpu = None
+    if not args.no_cpu_baseline:
+        try:
+            cpu = cpu_baseline(args)
+        except Exception as e:
+            cpu = {"error": f"{type(e).__name__}: {e}"}
     del flush, Vgs, outs
     # (N > 1: the other ranks are waiting at the final barrier; the report and the secondary workloads are in the N = 1 line)
-    parity = None if (args.no_parity or world > 1) else parity_report(args)
+    parity = None
+    if not (args.no_parity or world > 1):
+        try:
+            parity = parity_report(args)
+        except Exception as e:  # the report must never cost the headline line; an error here reads as "no parity claim"
+            parity = {"error": f"{type(e).__name__}: {e}"}
     secondary = None if (args.no_secondary or world > 1) else secondary_workloads(args, local_rank)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
