@@ -97,7 +97,6 @@ struct FoSort {  // thresholded: bookkeeping of the bucket sort and the walk
     unsigned short order[THR ? PIX : 1];   // pixel slots sorted by the number of free dots, descending
     unsigned char kfree[THR ? PIX : 1];    // number of free dots
     unsigned char wkey[THR ? PIX : 1];     // winning pattern
-    int bucket[16];
 };
 
 template <int N, bool THR, int PIX>
@@ -108,6 +107,8 @@ struct FoSmem {
     double nc[N][PIX];      // N_c of every pixel slot, parked during the walk (registers: 4 CTAs per SM)
     int32_t base[N][PIX];   // ... and the base point
     double cs[THR ? N : 1][PIX];     // thresholded: c_j of the compacted free dots, per pixel slot
+    int bucket[16];                  // thresholded: pixels of the CTA per number of free dots (outside the union below:
+                                     // zeroed before the first barrier)
     union {                    // C_gd is dead after S1 (a barrier separates it from the sort's first write)
         double CgT[QA_MAXG * N];   // CgT[k*N + i] = C_gd[i][k]
         FoSort<N, THR, PIX> sort;
@@ -262,6 +263,7 @@ __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel
     }
     for (int e = tid; e < N * g; e += FO_THREADS) sm.CgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
     for (int k = tid; k < (1 << N); k += FO_THREADS) sm.T[k] = mdl->QL[k];
+    if (THR && tid < 16) sm.bucket[tid] = 0;
     const int ns = mdl->ns;
     __syncthreads();
 
@@ -409,8 +411,6 @@ __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel
     } else {
         // compaction of the free dots (ascending bit position), bucket sort of the CTA's pixels by k, walk, hand back
         __syncthreads();  // every warp is done with C_gd: its storage becomes the sort's
-        if (tid < 16) sm.sort.bucket[tid] = 0;
-        __syncthreads();
 #pragma unroll
         for (int px = 0; px < FO_PX; ++px) {
             const int slot = px * FO_THREADS + tid;
@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel
             sm.sort.xm[slot] = xm;
             sm.sort.kfree[slot] = (unsigned char)kf;
             sm.sort.wkey[slot] = 0;
-            rk[px] = fo_bucket_rank(sm.sort.bucket, N - kf);
+            rk[px] = fo_bucket_rank(sm.bucket, N - kf);
         }
         __syncthreads();
 #pragma unroll
@@ -442,7 +442,7 @@ __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel
             int start = 0;
 #pragma unroll
             for (int bkt = 0; bkt <= N; ++bkt)
-                if (bkt < N - kf) start += sm.sort.bucket[bkt];
+                if (bkt < N - kf) start += sm.bucket[bkt];
             sm.sort.order[start + rk[px]] = (unsigned short)slot;
         }
         __syncthreads();
