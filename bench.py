@@ -254,12 +254,14 @@ def run_ours(args, rank, world, local_rank):
             for m_ in models:
                 m_.set_walk_variant(1)
 
-    pruned = mixed = None
+    pruned = mixed = one_kernel = None
     if args.workload == "config4":
         pruned = time_variant(2, "qa_model_set_walk_variant(2): high patterns excluded by a rigorous lower bound are not walked; "
                                  "identical N and E (tests/test_gpu_parity.py)")
         mixed = time_variant(3, "qa_model_set_walk_variant(3): pass 1 bounds every candidate from below in fp32 (directed rounding), "
                                 "pass 2 re-scores the survivors in fp64: N and E bit-identical to the fp64 walk")
+        one_kernel = time_variant(4, "qa_model_set_walk_variant(4): S1-S7 in one persistent kernel, no workspace traffic (DESIGN.md "
+                                     "section 5.4b); N, E and x bit-identical to the three launches")
         kw32 = mixed["kernel_times_ms"].get("qa_minplus_walk32_kernel", 0.0)
         if kw32 > 0:
             sm_count_ = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -341,7 +343,7 @@ def run_ours(args, rank, world, local_rank):
             "pixels_per_s": world * px_step / (ms_per_step * 1e-3), "diagram_ms": ms_per_step,
             "ms_per_step_min": float(times.min()), "ms_per_step_median": float(np.median(times)),
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-            "kernels_per_step": plan, "clocks": clocks, "pruned_variant": pruned, "mixed_precision_variant": mixed,
+            "kernels_per_step": plan, "clocks": clocks, "pruned_variant": pruned, "mixed_precision_variant": mixed, "one_kernel_variant": one_kernel,
             "parity": parity, "secondary": secondary,
             "paper_context": "paper: same diagram shape in < 1 s on a GTX 1080 Ti via JAX (PAPER.md L7, L498)"}
     print(json.dumps(line), flush=True)

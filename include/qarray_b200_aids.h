@@ -28,7 +28,10 @@ QA_API qa_status qa_get_kernel_timings(int max_kernels, float *ms, int *n_kernel
  * section 5, 2 = as 1, but the open default search of n_dot >= 13 skips the high patterns a rigorous lower bound excludes
  * (same arg min; fewer candidates are scored explicitly), 3 = as 1, but pass 1 of that search bounds every candidate in fp32
  * (packed adds, explicit error bound) and the fp64 pass 2 re-scores the threads the bound cannot exclude: charge map and
- * energies bit-identical to variant 1 (the "fp32 walk, fp64 re-score" path of SURVEY 8(f) NEXT-4).  Stored in the model (atomically); calls already enqueued are
+ * energies bit-identical to variant 1 (the "fp32 walk, fp64 re-score" path of SURVEY 8(f) NEXT-4), 4 = as 1, but the open
+ * default search of a 16-dot Maxwell array without sensor dots runs S1-S7 in ONE persistent kernel that touches no workspace
+ * (qa_minplus_fused_kernel; same arithmetic, bit-identical results; measured 4 % slower than the
+ * three launches, hence opt-in).  Stored in the model (atomically); calls already enqueued are
  * not affected.  Returns QA_ERR_INVALID_ARG for any other value.  The initial value of every model comes from the
  * environment variable QA_WALK_VARIANT (default 1). */
 QA_API qa_status qa_model_set_walk_variant(qa_model *model, int variant);

@@ -144,7 +144,8 @@ class Model:
     def set_walk_variant(self, variant: int):
         """qa_model_set_walk_variant (cross-check aid, qarray_b200_aids.h): 0 = three-kernel path with the exact-compare walk /
         generic enumeration everywhere, 1 = production dispatch, 2 = as 1 with exact pruning in the 13..16-dot min-plus walk,
-        3 = as 1 with the mixed-precision pass 1 (fp32 bound, fp64 re-score; bit-identical results)."""
+        3 = as 1 with the mixed-precision pass 1 (fp32 bound, fp64 re-score; bit-identical results), 4 = as 1 with the open
+        default search of 16 dots in one persistent kernel (no workspace traffic; bit-identical results)."""
         _check(lib().qa_model_set_walk_variant(self._h, int(variant)), "qa_model_set_walk_variant")
 
     def _check_device(self, Vg):

@@ -186,7 +186,7 @@ int initial_walk_variant()
 {
     const char *e = std::getenv("QA_WALK_VARIANT");
     const int v = e ? std::atoi(e) : 1;
-    return (v < 0 || v > 3) ? 1 : v;
+    return (v < 0 || v > 4) ? 1 : v;
 }
 
 // A model (batch) belongs to the device that was current when it was created.
@@ -282,6 +282,12 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     // open default search of 9..12 dots without sensor dots: the whole path in one kernel, a warp per two pixels
     if (!closed && alg == QA_ALG_DEFAULT && n > QA_FUSED_MAXN && n <= 12 && m->ns == 0 && variant != 0) {
         QA_CUDA(qa_launch_fused_mid(m->dev, n, m->walk, d_Vg, P, a, d_N, d_E, d_xcont, d_stats, stream));
+        timing_mark(stream);
+        return QA_OK;
+    }
+    // open default search of a 16-dot Maxwell array without sensor dots (variant 4): S1-S7 in one persistent kernel
+    if (!closed && alg == QA_ALG_DEFAULT && n == 16 && m->ns == 0 && m->is_z && variant == 4) {
+        QA_CUDA(qa_launch_minplus_fused(m->dev, m->host.QL, d_Vg, P, a, d_N, d_E, d_xcont, d_stats, m->sm_count, stream));
         timing_mark(stream);
         return QA_OK;
     }
@@ -751,7 +757,7 @@ qa_status qa_set_kernel_timing(int enable)
 
 qa_status qa_model_set_walk_variant(qa_model *m, int variant)
 {
-    if (!m || variant < 0 || variant > 3) return QA_ERR_INVALID_ARG;
+    if (!m || variant < 0 || variant > 4) return QA_ERR_INVALID_ARG;
     m->walk_variant.store(variant, std::memory_order_relaxed);
     return QA_OK;
 }

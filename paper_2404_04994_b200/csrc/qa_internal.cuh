@@ -91,6 +91,9 @@ cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const doubl
                                    double *d_E, int sm_count, int pruned, cudaStream_t stream);
 cudaError_t qa_launch_minplus_finish(const QaDevModel *d_model, int n, QaWorkspace ws, int32_t *d_N, double *d_E, unsigned slack,
                                      int sm_count, cudaStream_t stream);
+cudaError_t qa_launch_minplus_fused(const QaDevModel *d_model, const double *QLhost, const double *d_Vg, int64_t P, QaCallArgs args,
+                                    int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats, int sm_count,
+                                    cudaStream_t stream);
 cudaError_t qa_launch_minplus_walk32(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, int32_t *d_N,
                                      double *d_E, int sm_count, cudaStream_t stream);
 cudaError_t qa_launch_fused_mid(const QaDevModel *d_model, int n, const QaWalkTable &tab, const double *d_Vg, int64_t P,

@@ -39,6 +39,7 @@
 //
 // Index convention as in qa_kernels_walk.cu: candidate index = sum_i b_i 2^(n-1-i) = (t << NL) | (u << NW) | w.
 #include "qa_internal.cuh"
+#include "qa_prologue_lanes.cuh"
 
 namespace {
 
@@ -469,6 +470,124 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_pruned_kernel(con
 // one, whose inputs sit in shared memory; the survivor's constants (VT[t], QHT[t]) are read from the model tables the walk
 // kernel has just left in L2, lane i keeps row i of M in registers for S7, and each lane scores a block of CPL consecutive
 // candidates with a static add tree.
+// Pass 2 + S7 of ONE pixel by one warp (all 32 lanes call).  h: the pixel's h[0..N-1], E(base) (shared memory); r: the
+// record of walk warp `lane` (lanes < WPP); base_i, nc_i: base point and N_c of dot `lane` (lanes < N); ql: the lane's table
+// entries QL[lane * CPL ..]; mrow(j) = M[lane][j]; sd: N doubles of scratch of this warp.  outN == nullptr: only best[p].
+template <int NH, int NU, int NW, class MRow>
+__device__ __forceinline__ void mp_finish_pixel(const QaDevModel *__restrict__ mdl, const double *__restrict__ h, uint2 r,
+                                                int32_t base_i, double nc_i, const double2 (&ql)[(1 << (NU + NW - 5)) / 2],
+                                                double EC, unsigned slack, double *__restrict__ sd, MRow mrow, int64_t p,
+                                                uint64_t *__restrict__ best, int32_t *__restrict__ outN,
+                                                double *__restrict__ outE)
+{
+    constexpr int NL = NU + NW;
+    constexpr int N = NL + NH;
+    constexpr int WPP = (1 << NH) / 32;
+    constexpr int LB = NL - 5;          // log2 of the candidates per lane
+    constexpr int CPL = 1 << LB;        // candidates per lane: w = (wb << LB) + c, one u per lane
+    static_assert(LB >= 1 && LB <= NW, "a lane's block of candidates lies inside one u");
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned u = lane >> (NW - LB);                         // this lane's u
+    const unsigned wb = lane & ((1u << (NW - LB)) - 1u);          // ... and the bits of w above its block
+    const double e0 = h[N];
+    const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
+    const unsigned wmask = __ballot_sync(0xffffffffu, lane < (unsigned)WPP && r.x <= H + slack);  // warps that may hold the argmin
+
+    // thread-independent offsets, as pass 1 formed them (j ascending)
+    double offw = EC, offu = 0.0;
+#pragma unroll
+    for (int j = 0; j < NL; ++j) {
+        if (j < NW)
+            offw += fabs(h[N - 1 - j]);
+        else
+            offu += fabs(h[N - 1 - j]);
+    }
+
+    double bestE = INFINITY;
+    unsigned bestI = 0xffffffffu;
+    for (int q = 0; q < WPP; ++q) {
+        unsigned surv = __shfl_sync(0xffffffffu, r.y, q);
+        if (!((wmask >> q) & 1u)) continue;
+        while (surv) {
+            const unsigned ts = (unsigned)q * 32u + (unsigned)(__ffs(surv) - 1);
+            surv &= surv - 1;
+            // the survivor's inputs as pass 1 built them (same operands, same order)
+            double hp[NL];
+#pragma unroll
+            for (int j = 0; j < NL; ++j) hp[j] = h[N - 1 - j] + __ldg(mdl->VT + ts * NL + j);
+            double be = e0 + __ldg(mdl->QHT + ts);
+#pragma unroll
+            for (int jh = 0; jh < NH; ++jh)
+                if ((ts >> jh) & 1u) be += h[N - 1 - NL - jh];
+            // A[u] = ah[u >> 2] + lo[u & 3]
+            double a = be + offu;
+#pragma unroll
+            for (int j = NU - 1; j >= 2; --j)
+                if ((u >> j) & 1u) a += hp[NW + j];
+            if ((u & 3u) == 1u) a += hp[NW];
+            if ((u & 3u) == 2u) a += hp[NW + 1];
+            if ((u & 3u) == 3u) a += hp[NW + 1] + hp[NW];
+            // B[w] of the lane's block: bits of w from the highest down
+            double b[CPL];
+            b[0] = offw;
+#pragma unroll
+            for (int j = NW - 1; j >= LB; --j)
+                if ((wb >> (j - LB)) & 1u) b[0] += hp[j];
+#pragma unroll
+            for (int c = 1; c < CPL; ++c) b[c] = b[c & (c - 1)] + hp[mp_ctz(c)];
+            double e1 = INFINITY;
+            unsigned i1 = 0;
+#pragma unroll
+            for (int c = 0; c < CPL; c += 2) {
+                const double ea = a + (b[c] + ql[c >> 1].x), eb = a + (b[c + 1] + ql[c >> 1].y);
+                if (ea < e1) {  // c ascending within the lane: strict '<' keeps the smallest index
+                    e1 = ea;
+                    i1 = c;
+                }
+                if (eb < e1) {
+                    e1 = eb;
+                    i1 = c + 1;
+                }
+            }
+            i1 |= (ts << NL) | (lane << LB);
+            // lexicographic (e, index) minimum over the lanes.  Every e is positive (the offsets), so its bit pattern
+            // orders like its value: minimum of the high words, then of the low words among the lanes that hold it,
+            // then of the indices among those -- three warp reductions instead of five shuffle rounds.
+            const unsigned ehi = (unsigned)__double2hiint(e1), elo = (unsigned)__double2loint(e1);
+            const unsigned mhi = __reduce_min_sync(0xffffffffu, ehi);
+            const unsigned mlo = __reduce_min_sync(0xffffffffu, ehi == mhi ? elo : 0xffffffffu);
+            const bool tie = ehi == mhi && elo == mlo;
+            const unsigned mi = __reduce_min_sync(0xffffffffu, tie ? i1 : 0xffffffffu);
+            const double em = __hiloint2double((int)mhi, (int)mlo);
+            if (em < bestE || (em == bestE && mi < bestI)) {
+                bestE = em;
+                bestI = mi;
+            }
+        }
+    }
+    if (!outN) {
+        if (lane == 0) best[p] = (uint64_t)bestI;
+        return;
+    }
+    // S7: N* and E(N*) = 1/2 d^T M d from the definition (Eq. (C1)); lane i holds dot i and row i of M
+    int32_t Ni = 0;
+    double di = 0.0;
+    if (lane < (unsigned)N) {
+        Ni = base_i + (int32_t)((bestI >> (N - 1 - lane)) & 1u);
+        di = (double)Ni - nc_i;
+        sd[lane] = di;
+    }
+    __syncwarp();
+    double row = 0.0;
+#pragma unroll
+    for (int j = 0; j < N; ++j) row = fma(mrow(j), sd[j], row);
+    double E = di * row;  // lanes >= N hold di = 0
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) E += mp_shfl(E, (int)(lane ^ o));
+    if (lane < (unsigned)N) outN[p * N + lane] = Ni;
+    if (lane == 0) outE[p] = 0.5 * E;
+}
+
 template <int NH, int NU, int NW>
 __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaDevModel *__restrict__ mdl,
                                                                        QaWorkspace ws, int32_t *__restrict__ outN,
@@ -502,9 +621,6 @@ __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaD
     }
     qa_pdl_wait();  // model constants above; everything below was written by the prologue / walk kernels
 
-    const unsigned u = lane >> (NW - LB);                         // this lane's u
-    const unsigned wb = lane & ((1u << (NW - LB)) - 1u);          // ... and the bits of w above its block
-
     // inputs of a pixel, one value per lane
     double in_v = 0.0, in_nc = 0.0;
     int32_t in_base = 0;
@@ -527,105 +643,214 @@ __global__ void __launch_bounds__(MF_THREADS) qa_minplus_finish_kernel(const QaD
         __syncwarp();
         request(p + tw);
         const double *__restrict__ h = sIn[wid];
-        const double e0 = h[N];
-        const unsigned H = __reduce_min_sync(0xffffffffu, r.x);
-        const unsigned wmask = __ballot_sync(0xffffffffu, lane < (unsigned)WPP && r.x <= H + slack);  // warps that may hold the argmin
+        mp_finish_pixel<NH, NU, NW>(mdl, h, r, base_i, nc_i, ql, EC, slack, sd[wid], [&](int j) { return Mrow[j]; }, p, ws.best,
+                                    outN, outE);
+        __syncwarp();  // sIn / sd are rewritten by the next iteration
+    }
+}
 
-        // thread-independent offsets, as pass 1 formed them (j ascending)
-        double offw = EC, offu = 0.0;
+// ---------------------------------------------------------------------------------------------------------------------
+// The whole path S1-S7 of a 16-dot open array in ONE persistent kernel (NH = 8: a CTA of 256 threads = the 2^8 high
+// patterns of one pixel pair).  With three launches the step pays two launch gaps and two cold starts (prologue and finish
+// are ~15 us kernels that keep 2-20 % of the machine busy).  Here the walk of pixel pair `it` by all eight warps is pass 1
+// exactly as in qa_minplus_walk_kernel, and two small duties ride along in the issue slots the walk leaves idle:
+//   * the warp it % 8 first runs S1-S4 of pair it + LA (sixteen lanes per pixel: qa_prologue_lanes.cuh) into a
+//     shared-memory ring (h, E(base), base, N_c),
+//   * the warps (it + 3) % 8 and (it + 5) % 8 first run pass 2 + S7 (mp_finish_pixel) of the two pixels of pair it - FD from
+//     the ring (the eight warps left the records of that pair there).
+// There is no CTA barrier in the loop: a barrier per pair makes seven warps wait for the one that has a duty.  The warps
+// drift instead, and three counters per ring slot order the data (producer: data, fence, counter; consumer: counter,
+// fence, data): fIn = "inputs of pair j are in the slot", fRec = "warps that have left their record of pair j", fFin =
+// "pixels of pair j finished" (the slot may be refilled).  Every wait refers to work that other warps do in an EARLIER
+// iteration of theirs, so the waits are well-founded (no cycle); all warps of a CTA are resident, so they make progress.
+// Nothing but V_g is read from and nothing but N*, E(N*) (and x) is written to global memory; no workspace.
+__device__ __forceinline__ void mp_wait_eq(const unsigned *f, unsigned target)
+{
+    while (*reinterpret_cast<const volatile unsigned *>(f) != target) __nanosleep(40);
+    __threadfence_block();
+    __syncwarp();
+}
+__device__ __forceinline__ void mp_signal(unsigned *f, unsigned lane, unsigned value, bool add)
+{
+    __threadfence_block();
+    __syncwarp();
+    if (lane == 0) {
+        if (add)
+            atomicAdd(f, value);
+        else
+            *reinterpret_cast<volatile unsigned *>(f) = value;
+    }
+}
+
+template <int NU, int NW, int MINB>
+__global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_fused_kernel(const QaDevModel *__restrict__ mdl,
+                                                                            const __grid_constant__ MpTable<NU + NW> tab,
+                                                                            const double *__restrict__ Vg, int64_t P,
+                                                                            QaCallArgs args, int32_t *__restrict__ outN,
+                                                                            double *__restrict__ outE, double *__restrict__ xcont,
+                                                                            qa_stats *stats)
+{
+    constexpr int NH = 8, PX = 2, RING = 8, LA = 3, FD = 2;
+    constexpr int NL = NU + NW;
+    constexpr int N = NL + NH;
+    constexpr int WPP = 8;
+    constexpr int NCH = 1 << (NU - 2);
+    constexpr int CPL = 1 << (NL - 5);
+    static_assert(NL == QA_WALK_NL && N == 16 && MP_THREADS == 256, "one CTA = the 2^8 high patterns of a pixel pair");
+    static_assert(LA + FD < RING, "a slot is refilled only after its pair is finished");
+    __shared__ double sCgT[QA_MAXG * N], sC[N * N], sMT[N * N], sC1[N];
+    __shared__ double sV[WPP][PX][QA_MAXG], sX[WPP][PX][2 * N];  // scratch of the warp that runs S1-S4
+    __shared__ double sIn[RING][PX][N + 1], sNc[RING][PX][N];
+    __shared__ int32_t sBase[RING][PX][N];
+    __shared__ uint2 sRec[RING][PX][WPP];
+    __shared__ double sd[WPP][N];
+    __shared__ unsigned fIn[RING], fRec[RING], fFin[RING];
+
+    const int tid = threadIdx.x;
+    const unsigned lane = tid & 31u;
+    const unsigned t = tid;
+    const int wid = tid >> 5;
+    const int g = mdl->g;
+    for (int e = tid; e < N * N; e += MP_THREADS) {
+        sMT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
+        sC[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
+    }
+    for (int e = tid; e < N * g; e += MP_THREADS) sCgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
+    if (tid < N) sC1[tid] = mdl->C1[tid];
+    if (tid < RING) fIn[tid] = fRec[tid] = fFin[tid] = 0u;
+    double v[NL];
 #pragma unroll
-        for (int j = 0; j < NL; ++j) {
-            if (j < NW)
-                offw += fabs(h[N - 1 - j]);
-            else
-                offu += fabs(h[N - 1 - j]);
+    for (int j = 0; j < NL; ++j) v[j] = mdl->VT[t * NL + j];
+    const double EC = mdl->EC;
+    const double QH = mdl->QHT[t];
+    __syncthreads();
+
+    const int64_t groups = (P + PX - 1) / PX;
+    // (the launcher keeps the pairs per CTA below 2^30: 32-bit loop control)
+    const int nit = blockIdx.x < groups ? (int)((groups - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    int64_t st_np = 0, st_nq = 0, st_nr = 0, st_nf = 0;
+
+    // S1-S4 of pixel pair j by the calling warp (sixteen lanes per pixel) into ring slot j % RING
+    auto prologue = [&](int j) {
+        const int64_t grp = blockIdx.x + j * (int64_t)gridDim.x;
+        const int s = (int)(lane >> 4), i = (int)(lane & 15u), gb = (int)(lane & 16u);
+        const int64_t p = grp * PX + s;
+        const bool live = p < P;
+        const int64_t pp = live ? p : P - 1;
+        const int slot = j & (RING - 1);
+        mp_wait_eq(&fFin[slot], (unsigned)(PX * (j / RING)));  // the pair that used the slot before is finished
+        for (int k = i; k < g; k += 16) sV[wid][s][k] = __ldg(Vg + pp * g + k);
+        __syncwarp();
+        QaLaneOut lo;
+        qa_lanes_pixel<N>(sCgT, sC, sMT, sC1, 1.0, sV[wid][s], sX[wid][s], g, i, gb, true, args, lo);
+        sIn[slot][s][i] = lo.gi + 0.5 * sMT[i * N + i];
+        if (i == 0) sIn[slot][s][N] = 0.5 * lo.e0;
+        sNc[slot][s][i] = lo.nc;
+        sBase[slot][s][i] = lo.base;
+        if (live && xcont) xcont[p * N + i] = lo.x;
+        if (live && i == 0) {
+            ++st_np;
+            st_nq += lo.neg0 != 0u ? 1 : 0;
+            st_nr += lo.rounds;
+            st_nf += lo.failed ? 1 : 0;
         }
+        mp_signal(&fIn[slot], lane, (unsigned)(j + 1), false);
+    };
+    if (wid < LA && wid < nit) prologue(wid);
 
-        double bestE = INFINITY;
-        unsigned bestI = 0xffffffffu;
-        for (int q = 0; q < WPP; ++q) {
-            unsigned surv = __shfl_sync(0xffffffffu, r.y, q);
-            if (!((wmask >> q) & 1u)) continue;
-            while (surv) {
-                const unsigned ts = (unsigned)q * 32u + (unsigned)(__ffs(surv) - 1);
-                surv &= surv - 1;
-                // the survivor's inputs as pass 1 built them (same operands, same order)
-                double hp[NL];
+    for (int it = 0; it < nit + FD; ++it) {
+        // ---- duty: S1-S4 of a pair ahead
+        if (it + LA < nit && wid == (it & 7)) prologue(it + LA);
+        // ---- duty: pass 2 + S7 of a pair behind
+        if (it >= FD) {
+            const int px = wid == ((it + 3) & 7) ? 0 : (wid == ((it + 5) & 7) ? 1 : -1);
+            if (px >= 0) {
+                const int j = it - FD;
+                const int slot = j & (RING - 1);
+                const int64_t p = (blockIdx.x + j * (int64_t)gridDim.x) * PX + px;
+                mp_wait_eq(&fRec[slot], (unsigned)(WPP * (j / RING + 1)));  // all eight warps have left their record
+                if (p < P) {
+                    const uint2 r = lane < (unsigned)WPP ? sRec[slot][px][lane] : make_uint2(0xffffffffu, 0u);
+                    const int li = lane < (unsigned)N ? (int)lane : 0;
+                    double2 ql[CPL / 2];
 #pragma unroll
-                for (int j = 0; j < NL; ++j) hp[j] = h[N - 1 - j] + __ldg(mdl->VT + ts * NL + j);
-                double be = e0 + __ldg(mdl->QHT + ts);
-#pragma unroll
-                for (int jh = 0; jh < NH; ++jh)
-                    if ((ts >> jh) & 1u) be += h[N - 1 - NL - jh];
-                // A[u] = ah[u >> 2] + lo[u & 3]
-                double a = be + offu;
-#pragma unroll
-                for (int j = NU - 1; j >= 2; --j)
-                    if ((u >> j) & 1u) a += hp[NW + j];
-                if ((u & 3u) == 1u) a += hp[NW];
-                if ((u & 3u) == 2u) a += hp[NW + 1];
-                if ((u & 3u) == 3u) a += hp[NW + 1] + hp[NW];
-                // B[w] of the lane's block: bits of w from the highest down
-                double b[CPL];
-                b[0] = offw;
-#pragma unroll
-                for (int j = NW - 1; j >= LB; --j)
-                    if ((wb >> (j - LB)) & 1u) b[0] += hp[j];
-#pragma unroll
-                for (int c = 1; c < CPL; ++c) b[c] = b[c & (c - 1)] + hp[mp_ctz(c)];
-                double e1 = INFINITY;
-                unsigned i1 = 0;
-#pragma unroll
-                for (int c = 0; c < CPL; c += 2) {
-                    const double ea = a + (b[c] + ql[c >> 1].x), eb = a + (b[c + 1] + ql[c >> 1].y);
-                    if (ea < e1) {  // c ascending within the lane: strict '<' keeps the smallest index
-                        e1 = ea;
-                        i1 = c;
-                    }
-                    if (eb < e1) {
-                        e1 = eb;
-                        i1 = c + 1;
-                    }
+                    for (int c = 0; c < CPL / 2; ++c) ql[c] = __ldg(reinterpret_cast<const double2 *>(mdl->QL + lane * CPL) + c);
+                    mp_finish_pixel<NH, NU, NW>(mdl, sIn[slot][px], r, sBase[slot][px][li], sNc[slot][px][li], ql, EC, 2u, sd[wid],
+                                                [&](int jj) { return sMT[jj * N + li]; }, p, nullptr, outN, outE);
                 }
-                i1 |= (ts << NL) | (lane << LB);
-                // lexicographic (e, index) minimum over the lanes.  Every e is positive (the offsets), so its bit pattern
-                // orders like its value: minimum of the high words, then of the low words among the lanes that hold it,
-                // then of the indices among those -- three warp reductions instead of five shuffle rounds.
-                const unsigned ehi = (unsigned)__double2hiint(e1), elo = (unsigned)__double2loint(e1);
-                const unsigned mhi = __reduce_min_sync(0xffffffffu, ehi);
-                const unsigned mlo = __reduce_min_sync(0xffffffffu, ehi == mhi ? elo : 0xffffffffu);
-                const bool tie = ehi == mhi && elo == mlo;
-                const unsigned mi = __reduce_min_sync(0xffffffffu, tie ? i1 : 0xffffffffu);
-                const double em = __hiloint2double((int)mhi, (int)mlo);
-                if (em < bestE || (em == bestE && mi < bestI)) {
-                    bestE = em;
-                    bestI = mi;
-                }
+                mp_signal(&fFin[slot], lane, 1u, true);
             }
         }
-        if (!outN) {
-            if (lane == 0) ws.best[p] = (uint64_t)bestI;
-            __syncwarp();
-            continue;
-        }
-        // S7: N* and E(N*) = 1/2 d^T M d from the definition (Eq. (C1)); lane i holds dot i and row i of M
-        int32_t Ni = 0;
-        double di = 0.0;
-        if (lane < (unsigned)N) {
-            Ni = base_i + (int32_t)((bestI >> (N - 1 - lane)) & 1u);
-            di = (double)Ni - nc_i;
-            sd[wid][lane] = di;
-        }
-        __syncwarp();
-        double row = 0.0;
+        // ---- pass 1 of pair `it`: qa_minplus_walk_kernel's arithmetic, inputs from the ring
+        if (it < nit) {
+            const int slot = it & (RING - 1);
+            mp_wait_eq(&fIn[slot], (unsigned)(it + 1));
+            double B[PX][1 << NW], hu[PX][NU], a0[PX], lo3[PX];
 #pragma unroll
-        for (int j = 0; j < N; ++j) row = fma(Mrow[j], sd[wid][j], row);
-        double E = di * row;  // lanes >= N hold di = 0
+            for (int px = 0; px < PX; ++px) {
+                const double *__restrict__ hin = sIn[slot][px];
+                double hw[NW], offw = EC, offu = 0.0;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) E += mp_shfl(E, (int)(lane ^ o));
-        if (lane < (unsigned)N) outN[p * N + lane] = Ni;
-        if (lane == 0) outE[p] = 0.5 * E;
-        __syncwarp();  // sIn / sd are rewritten by the next iteration
+                for (int j = 0; j < NL; ++j) {
+                    const double hj = hin[N - 1 - j];
+                    if (j < NW) {
+                        hw[j] = hj + v[j];
+                        offw += fabs(hj);
+                    } else {
+                        hu[px][j - NW] = hj + v[j];
+                        offu += fabs(hj);
+                    }
+                }
+                double be = hin[N] + QH;
+#pragma unroll
+                for (int jh = 0; jh < NH; ++jh) {
+                    const double hv = hin[N - 1 - NL - jh];
+                    if ((t >> jh) & 1u) be += hv;
+                }
+                a0[px] = be + offu;
+                lo3[px] = hu[px][1] + hu[px][0];
+                B[px][0] = offw;
+#pragma unroll
+                for (int w = 1; w < (1 << NW); ++w) B[px][w] = B[px][w & (w - 1)] + hw[mp_ctz(w)];
+            }
+            unsigned L[PX];
+#pragma unroll
+            for (int px = 0; px < PX; ++px) L[px] = 0xffffffffu;
+            int iv;
+            asm volatile("mov.u32 %0, 0;" : "=r"(iv));
+#pragma unroll 1
+            for (int i = 0; i < NCH; ++i, ++iv) {
+                const double2 *q = reinterpret_cast<const double2 *>(tab.q) + (i << (NW + 1));
+                double a[4][PX];
+#pragma unroll
+                for (int px = 0; px < PX; ++px) {
+                    double ah = a0[px];
+#pragma unroll
+                    for (int j = NU - 1; j >= 2; --j)
+                        if ((iv >> (j - 2)) & 1) ah += hu[px][j];
+                    a[0][px] = ah;
+                    a[1][px] = ah + hu[px][0];
+                    a[2][px] = ah + hu[px][1];
+                    a[3][px] = ah + lo3[px];
+                }
+                mp_chunk<NW, PX>(q, B, a, L);
+            }
+#pragma unroll
+            for (int px = 0; px < PX; ++px) {
+                const unsigned wmin = __reduce_min_sync(0xffffffffu, L[px]);
+                const unsigned ball = __ballot_sync(0xffffffffu, L[px] <= wmin + 2u);
+                if (lane == 0) sRec[slot][px][wid] = make_uint2(wmin, ball);
+            }
+            mp_signal(&fRec[slot], lane, 1u, true);
+        }
+    }
+    if (stats) {
+        qa_warp_count(&stats->n_pixels, st_np);
+        qa_warp_count(&stats->n_qp_pixels, st_nq);
+        qa_warp_count(&stats->n_qp_rounds, st_nr);
+        qa_warp_count(&stats->n_qp_failed, st_nf);
+        qa_warp_count(&stats->n_candidates_enumerated, st_np << N);
+        qa_warp_count(&stats->n_candidates_scored, st_np << N);
     }
 }
 
@@ -730,4 +955,25 @@ cudaError_t qa_launch_minplus_finish(const QaDevModel *d_model, int n, QaWorkspa
         case 16: return launch_finish<8, 4, 4>(d_model, ws, d_N, d_E, sm_count, stream, slack);
         default: return cudaErrorInvalidValue;
     }
+}
+
+// Open default search of a 16-dot Maxwell array without sensor dots: the whole path in one persistent kernel.
+cudaError_t qa_launch_minplus_fused(const QaDevModel *d_model, const double *QLhost, const double *d_Vg, int64_t P, QaCallArgs args,
+                                    int32_t *d_N, double *d_E, double *d_xcont, qa_stats *d_stats, int sm_count,
+                                    cudaStream_t stream)
+{
+    qa_plan_add("qa_minplus_fused_kernel");
+    MpTable<8> local;
+    for (int b = 0; b < 256; ++b) local.q[b] = QLhost[b];
+    int per_sm = 0;
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_fused_kernel<4, 4, 2>, MP_THREADS, 0);
+    if (err != cudaSuccess) return err;
+    if (per_sm < 1) per_sm = 1;
+    int64_t grid = (int64_t)sm_count * per_sm;
+    const int64_t need = (P + 1) / 2;
+    if (grid > need) grid = need;
+    if (need / grid >= ((int64_t)1 << 30)) return cudaErrorInvalidValue;  // (P <= 2^40: only with a grid below 512 CTAs)
+    qa_minplus_fused_kernel<4, 4, 2><<<(unsigned)grid, MP_THREADS, 0, stream>>>(d_model, local, d_Vg, P, args, d_N, d_E, d_xcont,
+                                                                               d_stats);
+    return cudaGetLastError();
 }

@@ -165,18 +165,22 @@ def full_size_report(api, oracle, wl, torch, strict=False, config5_members=256, 
         om = oracle.Model(w.C_dd, w.C_gd)
         o = om.ground_state(w.Vg, n_threads=nt)
         rs = []
-        for variant in (1, 2, 0, 3):
+        for variant in (1, 2, 0, 3, 4):
             g = _gpu(api, torch, w, variant=variant)
             rs.append(compare(g["N"], g["E"], o, om.EC, g["xcont"], strict=strict))
             if variant == 1:
                 g1 = g
-        r_mixed_equal = bool(np.array_equal(g["N"], g1["N"]) and np.array_equal(g["E"], g1["E"]))
+            if variant == 3:
+                g3 = g
+        r_mixed_equal = bool(np.array_equal(g3["N"], g1["N"]) and np.array_equal(g3["E"], g1["E"]))
+        r_fused_equal = bool(np.array_equal(g["N"], g1["N"]) and np.array_equal(g["E"], g1["E"]))
         r = dict(rs[0])
         for k in ("mismatch", "excused_near_tie", "unexcused", "E_out_of_tolerance"):
             r[k + "_all_variants"] = int(sum(x[k] for x in rs))
         r["mixed_precision_walk_bit_identical_to_fp64_walk"] = r_mixed_equal
+        r["one_kernel_path_bit_identical_to_fp64_walk"] = r_fused_equal
         r.update(algorithms="default; walk variants 1 (min-plus), 2 (pruned), 0 (exact-compare walk), 3 (fp32 lower-bound pass + "
-                            "fp64 re-score), each vs the oracle",
+                            "fp64 re-score), 4 (S1-S7 in one persistent kernel), each vs the oracle",
                  oracle_s=round(time.perf_counter() - t0, 2))
         rep["config4"] = r
     if 5 in configs:

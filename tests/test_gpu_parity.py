@@ -141,8 +141,11 @@ def test_walk_variants_agree(api, n, P):
     plans = {0: ["qa_prologue_kernel", "qa_walk_kernel", "qa_finalize_kernel"],
              1: ["qa_prologue_lanes_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"],
              2: ["qa_prologue_lanes_kernel", "qa_minplus_pruned_kernel", "qa_minplus_finish_kernel"],
-             3: ["qa_prologue_lanes_kernel", "qa_minplus_walk32_kernel", "qa_minplus_finish_kernel"]}
-    for variant in (0, 1, 2, 3):
+             3: ["qa_prologue_lanes_kernel", "qa_minplus_walk32_kernel", "qa_minplus_finish_kernel"],
+             # variant 4: S1-S7 in one persistent kernel (16 dots only; other sizes run as variant 1)
+             4: ["qa_minplus_fused_kernel"] if n == 16 else
+                ["qa_prologue_lanes_kernel", "qa_minplus_walk_kernel", "qa_minplus_finish_kernel"]}
+    for variant in (0, 1, 2, 3, 4):
         rep, g, o = check(api, w, variant=variant, algorithm="default")
         assert g["plan"][0] == plans[variant]
         if ref is None:
@@ -162,7 +165,7 @@ def test_minplus_walk_many_groups_per_worker(api, n, P):
     om = oracle.Model(w.C_dd, w.C_gd)
     o = om.ground_state(w.Vg, n_threads=os.cpu_count() or 1)
     ref = None
-    for variant in (0, 1, 2, 3):
+    for variant in (0, 1, 2, 3, 4):
         g = run_gpu(api, w, variant=variant)
         compare(g["N"], g["E"], o, om.EC, gpu_x=g["xcont"])
         assert g["stats"]["n_qp_pixels"] == int(((o["flags"] & oracle.FLAG_QP) != 0).sum()) and g["stats"]["n_qp_failed"] == 0
@@ -185,13 +188,15 @@ def test_minplus_walks_against_exact_walk_many_models(api, n):
         _, EC = m.inverse()
         Vg = torch.from_numpy(w.Vg).cuda()
         outs = {}
-        for variant in (0, 1, 2, 3):
+        for variant in (0, 1, 2, 3, 4):
             m.set_walk_variant(variant)
             r = m.ground_state(Vg)
             torch.cuda.synchronize()
             outs[variant] = (r["N"].cpu().numpy(), r["E"].cpu().numpy())
-        # the mixed-precision walk (fp32 lower bound, fp64 exact re-score) must reproduce the fp64 walk bit for bit
-        assert np.array_equal(outs[3][0], outs[1][0]) and np.array_equal(outs[3][1], outs[1][1])
+        # the mixed-precision walk (fp32 lower bound, fp64 exact re-score) must reproduce the fp64 walk bit for bit, and so
+        # must the one-kernel path (same arithmetic, inputs through shared memory instead of the workspace)
+        for variant in (3, 4):
+            assert np.array_equal(outs[variant][0], outs[1][0]) and np.array_equal(outs[variant][1], outs[1][1])
         for variant in (1, 2):
             diff = (outs[variant][0] != outs[0][0]).any(1)
             assert np.abs(outs[variant][1] - outs[0][1])[diff].max(initial=0.0) <= 1e-9 * EC
@@ -206,7 +211,7 @@ def test_minplus_walk_extreme_inputs(api):
     rng = np.random.default_rng(7)
     Vg = np.concatenate([w.Vg, -50.0 * np.abs(rng.standard_normal((7, 16))), w.Vg[:9] * 40.0, np.zeros((3, 16))])
     w.Vg, w.W, w.H = np.ascontiguousarray(Vg), Vg.shape[0], 1
-    for variant in (0, 1, 2, 3):
+    for variant in (0, 1, 2, 3, 4):
         check(api, w, variant=variant, algorithm="default")
 
 
