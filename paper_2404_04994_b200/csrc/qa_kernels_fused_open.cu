@@ -213,7 +213,7 @@ __device__ __forceinline__ int fo_bucket_rank(int *bucket, int key)
     return start + __popc(peers & ((1u << lane) - 1u));
 }
 
-template <int N, bool THR, int PX>
+template <int N, bool THR, int PX, bool MP>
 __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel(const QaDevModel *const *__restrict__ models,
                                                                    const double *__restrict__ Vg, int64_t P, int g,
                                                                    QaCallArgs args, int32_t *__restrict__ outN,
@@ -265,6 +265,7 @@ __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel
     for (int k = tid; k < (1 << N); k += FO_THREADS) sm.T[k] = mdl->QL[k];
     if (THR && tid < 16) sm.bucket[tid] = 0;
     const int ns = mdl->ns;
+    const double EC = MP ? mdl->EC : 0.0;
     __syncthreads();
 
     // ---- S1-S4
@@ -352,7 +353,101 @@ __global__ void __launch_bounds__(FO_THREADS, 4 * (3 - PX)) qa_fused_open_kernel
     asm volatile("" ::: "memory");
     // ---- S5-S6
     unsigned win[FO_PX];
-    if constexpr (!THR) {
+    if constexpr (!THR && MP) {
+        // Maxwell c_dd (pair energies >= 0), N >= 5: the min-plus split of qa_kernels_minplus.cu inside one thread.  With
+        // w = bits [0,4), u = bits [4,N):  e(u,w) = A[u] + (B[w] + T[u,w]),  B[w] = offW + sum_{j in w} h'_j,
+        // A[u] = offU + sum_{j in u} h'_j,  offW = E_C + sum_{j<4} |h'_j|, offU = E_C + sum_{j>=4} |h'_j| (every y = B + T and
+        // every A is positive: the high 32 bits of the patterns order like the values).
+        //   pass 1:  m_u = min_w hi32(y)  (one DADD + half an integer min3 per candidate),  L_u = hi32(A[u] + double(m_u, 0))
+        //            is a lower bound of the row's energies, and the row of the arg min (and of every tie) has
+        //            L_u <= min L + 2 (qa_kernels_minplus.cu header).  Rows are taken four at a time in a real loop; per
+        //            group the minimum and the rows within 2 of it are kept (a superset of the rows within 2 of min L).
+        //   pass 2:  the rows that can hold the arg min (1.2 on average) are scored with the same arithmetic and the exact
+        //            compare, ascending index: the lexicographically smallest N among equal energies (reading R6).
+        // 1.3 FP64 instructions per candidate instead of 3, and no dependent chain through the running sum.
+        constexpr int NW = 4, NU = N - NW, R = 1 << NU, GS = R < 4 ? R : 4, NG = R / GS;
+        static_assert(N > NW, "at least one high bit");
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            double B[1 << NW], hu[NU];
+            double offw = EC, offu = EC;
+#pragma unroll
+            for (int j = 0; j < NW; ++j) offw += fabs(hp[px][j]);
+#pragma unroll
+            for (int j = 0; j < NU; ++j) {
+                hu[j] = hp[px][NW + j];
+                offu += fabs(hu[j]);
+            }
+            B[0] = offw;
+#pragma unroll
+            for (int w = 1; w < (1 << NW); ++w) B[w] = B[w & (w - 1)] + hp[px][fo_ctz(w)];
+            const double lo3 = NU >= 2 ? hu[NU >= 2 ? 1 : 0] + hu[0] : 0.0;
+            // A[u] of row u = 4 i + ul (the same expression in both passes: bitwise the same value)
+            auto row_a = [&](int i, int ul) -> double {
+                double ah = offu;
+#pragma unroll
+                for (int j = NU - 1; j >= 2; --j)
+                    if ((i >> (j - 2)) & 1) ah += hu[j];
+                if (NU >= 2) return ul == 0 ? ah : (ul == 1 ? ah + hu[0] : (ul == 2 ? ah + hu[NU >= 2 ? 1 : 0] : ah + lo3));
+                return ul == 0 ? ah : ah + hu[0];
+            };
+            unsigned Lg[NG], rowmask = 0;
+#pragma unroll
+            for (int k = 0; k < NG; ++k) Lg[k] = 0xffffffffu;
+#pragma unroll 1
+            for (int i = 0; i < NG; ++i) {
+                const double2 *__restrict__ T2 = reinterpret_cast<const double2 *>(sm.T + ((i * GS) << NW));
+                unsigned l[GS];
+#pragma unroll
+                for (int ul = 0; ul < GS; ++ul) {
+                    unsigned m0 = 0xffffffffu, m1 = 0xffffffffu;
+#pragma unroll
+                    for (int w = 0; w < (1 << NW); w += 4) {
+                        const double2 ta = T2[((ul << NW) | w) >> 1], tb = T2[((ul << NW) | (w + 2)) >> 1];
+                        const double y0 = B[w] + ta.x, y1 = B[w + 1] + ta.y, y2 = B[w + 2] + tb.x, y3 = B[w + 3] + tb.y;
+                        m0 = min(m0, min((unsigned)__double2hiint(y0), (unsigned)__double2hiint(y1)));
+                        m1 = min(m1, min((unsigned)__double2hiint(y2), (unsigned)__double2hiint(y3)));
+                    }
+                    const double lb = row_a(i, ul) + __hiloint2double((int)min(m0, m1), 0);
+                    l[ul] = (unsigned)__double2hiint(lb);
+                }
+                unsigned gmin = l[0];
+#pragma unroll
+                for (int ul = 1; ul < GS; ++ul) gmin = min(gmin, l[ul]);
+                unsigned nib = 0;
+#pragma unroll
+                for (int ul = 0; ul < GS; ++ul) nib |= (l[ul] <= gmin + 2u ? 1u : 0u) << ul;
+                rowmask |= nib << (i * GS);
+#pragma unroll
+                for (int k = 0; k < NG; ++k)
+                    if (k == i) Lg[k] = gmin;
+            }
+            unsigned Lmin = Lg[0];
+#pragma unroll
+            for (int k = 1; k < NG; ++k) Lmin = min(Lmin, Lg[k]);
+            unsigned cand = 0;
+#pragma unroll
+            for (int k = 0; k < NG; ++k)
+                if (Lg[k] <= Lmin + 2u) cand |= rowmask & (((1u << GS) - 1u) << (k * GS));
+            double best = __longlong_as_double(0x7ff0000000000000ll);
+            unsigned bkey = 0;
+            while (cand) {
+                const int u = __ffs(cand) - 1;
+                cand &= cand - 1u;
+                const double a = row_a(u / GS, u % GS);
+                const double *__restrict__ T = sm.T + (u << NW);
+#pragma unroll
+                for (int w = 0; w < (1 << NW); ++w) {
+                    const double e = a + (B[w] + T[w]);
+                    if (e < best) {
+                        best = e;
+                        bkey = ((unsigned)u << NW) | (unsigned)w;
+                    }
+                }
+            }
+            win[px] = bkey;
+        }
+    } else if constexpr (!THR) {
         // counting-order walk over all 2^N patterns, both pixels at once (qa_kernels_walk.cu).  A real loop over chunks of
         // 2^LB patterns (the fully unrolled walk is 60 KB of code and stalls on instruction fetch): inside a chunk every
         // index is static; the step into chunk i sets bit LB + ctz(i), picked from registers by a short select chain.
@@ -564,12 +659,17 @@ cudaError_t launch_fused_open_n(const QaDevModel *const *d_models, int n_models,
                                 qa_stats *d_stats, cudaStream_t stream)
 {
     const dim3 grid((unsigned)((P + FO_THREADS * FO_PX_RUN - 1) / (FO_THREADS * FO_PX_RUN)), (unsigned)n_models);
-    if (args.alg == QA_ALG_DEFAULT)
-        qa_fused_open_kernel<N, false, FO_PX_RUN><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont,
-                                                                                d_Vs, d_stats);
-    else
-        qa_fused_open_kernel<N, true, FO_PX_RUN><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E, d_xcont,
-                                                                               d_Vs, d_stats);
+    if (args.alg == QA_ALG_DEFAULT) {
+        // Maxwell models (every model of the call) with at least five dots: the min-plus form of the walk
+        if (N >= 5 && args.general_qp == 0)
+            qa_fused_open_kernel<N, false, FO_PX_RUN, (N >= 5)><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E,
+                                                                                              d_xcont, d_Vs, d_stats);
+        else
+            qa_fused_open_kernel<N, false, FO_PX_RUN, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E,
+                                                                                           d_xcont, d_Vs, d_stats);
+    } else
+        qa_fused_open_kernel<N, true, FO_PX_RUN, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, args, d_N, d_E,
+                                                                                      d_xcont, d_Vs, d_stats);
     return cudaGetLastError();
 }
 
