@@ -49,7 +49,8 @@ typedef enum {
     QA_ERR_INFEASIBLE = 5,       /* closed array: N_hat < 0, or brute force with n_dot * n_max < N_hat                 */
     QA_ERR_OVERFLOW = 6,         /* brute force: (n_max + 1)^n_dot >= 2^62                                             */
     QA_ERR_CUDA = 7,             /* a CUDA runtime call failed; see qa_last_cuda_error()                               */
-    QA_ERR_UNSUPPORTED = 8       /* reserved (earlier versions refused a c_dd with a positive off-diagonal entry)      */
+    QA_ERR_UNSUPPORTED = 8,      /* reserved (earlier versions refused a c_dd with a positive off-diagonal entry)      */
+    QA_ERR_STATIC_WORKSPACE = 9  /* qa_ground_state_open_static: the sweep needs more scratch than the static array     */
 } qa_status;
 
 /* The three candidate sets of the paper (Table I). */
@@ -121,6 +122,32 @@ QA_API size_t qa_workspace_bytes(const qa_model *model, int64_t P);
 QA_API qa_status qa_ground_state_open(const qa_model *model, const double *d_Vg, int64_t P, qa_algorithm alg, double t,
                                int n_max, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor,
                                qa_stats *d_stats, void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* ---- the same search without any allocation on the caller's side ---------------------------------------------------- */
+
+/* qa_ground_state_open for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid allocation): identical arguments, kernels and results, but the workspace is a file-scope
+ * `static __device__` array inside the library of QA_STATIC_WORKSPACE_BYTES (16 MiB; every GPU that loads the library holds
+ * it until the process exits) instead of a buffer the caller allocates.
+ *   - Limit: qa_workspace_bytes(model, P) <= QA_STATIC_WORKSPACE_BYTES, i.e. P <= 25 000 pixels at 16 dots (664 bytes per
+ *     pixel; a 100x100 diagram needs 6.7 MB), more for smaller arrays.  A larger sweep is rejected with
+ *     QA_ERR_STATIC_WORKSPACE before anything is enqueued; qa_static_workspace_last_error() says how much was needed.
+ *   - Every call on a device shares the one array, which keeps the previous call's contents.  Nothing in it has to start at
+ *     zero except the work counter of the pruned walk, which the first kernel of every call zeroes itself.  Calls that
+ *     OVERLAP on the GPU (different streams or host threads, same device) race on the array: the caller serialises them
+ *     (same stream, or an event between them).
+ *   - The device address of the array is fetched once per device (cudaGetSymbolAddress, with that device current) at the
+ *     first call on that device, or ahead of time by qa_static_workspace_init() -- call it once, with the device current,
+ *     before a stream capture begins.  The call itself calls no cudaMalloc / cudaFree / allocating library routine (with
+ *     the kernel-timing aid of qarray_b200_aids.h off).
+ * Other arguments, stream semantics and errors as qa_ground_state_open. */
+#define QA_STATIC_WORKSPACE_BYTES ((size_t)16 << 20)
+QA_API size_t qa_static_workspace_bytes(void); /* = QA_STATIC_WORKSPACE_BYTES */
+QA_API qa_status qa_static_workspace_init(void);
+QA_API const char *qa_static_workspace_last_error(void); /* text of this host thread's last failure of the calls above/below */
+QA_API qa_status qa_ground_state_open_static(const qa_model *model, const double *d_Vg, int64_t P, qa_algorithm alg, double t,
+                                             int n_max, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vsensor,
+                                             qa_stats *d_stats, void *cuda_stream);
 
 /* Closed array: additionally (iii) sum_i N_i = N_hat (L54-L56).  Paper API: ground_state_closed(vg, n_charges) (L454).
  * Candidates with the wrong total are eliminated (L127, L159); thresholded: per-pixel threshold doubling (L141, R5). */

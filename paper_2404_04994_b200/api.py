@@ -19,14 +19,15 @@ QA_OK = 0
 QA_ALG_DEFAULT, QA_ALG_THRESHOLDED, QA_ALG_BRUTE_FORCE = 0, 1, 2
 ALG = {"default": 0, "thresholded": 1, "brute": 2, "brute_force": 2}
 STATUS_NAMES = ["QA_OK", "QA_ERR_INVALID_ARG", "QA_ERR_NOT_SYMMETRIC", "QA_ERR_NOT_POSDEF", "QA_ERR_UNSUPPORTED_SIZE",
-                "QA_ERR_INFEASIBLE", "QA_ERR_OVERFLOW", "QA_ERR_CUDA", "QA_ERR_UNSUPPORTED"]
+                "QA_ERR_INFEASIBLE", "QA_ERR_OVERFLOW", "QA_ERR_CUDA", "QA_ERR_UNSUPPORTED", "QA_ERR_STATIC_WORKSPACE"]
 EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "qa_model_n_dot", "qa_model_n_gate",
            "qa_model_n_sensor", "qa_model_n_search", "qa_model_get_inverse", "qa_workspace_bytes", "qa_ground_state_open",
            "qa_ground_state_closed", "qa_ground_state_host", "qa_measure_fp64_rate", "qa_set_kernel_timing",
            "qa_get_kernel_timings", "qa_model_set_walk_variant", "qa_batch_create", "qa_batch_destroy", "qa_batch_size",
            "qa_ground_state_batch", "qa_thermal_open", "qa_thermal_closed", "qa_sensor_response",
            "qa_sensor_response_workspace_bytes", "qa_last_launch_plan",
-           "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version"]
+           "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version", "qa_static_workspace_bytes",
+           "qa_static_workspace_init", "qa_static_workspace_last_error", "qa_ground_state_open_static"]
 
 
 class qa_stats(C.Structure):
@@ -61,6 +62,8 @@ class QaError(RuntimeError):
         name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
         msg = lib().qa_status_string(status).decode()
         extra = lib().qa_last_cuda_error().decode() if status == 7 else ""
+        if status == 9 or "static" in where:
+            extra = (extra + " " + lib().qa_static_workspace_last_error().decode()).strip()
         super().__init__(f"{where}: {name} ({msg}) {extra}".strip())
 
 
@@ -86,6 +89,9 @@ def lib() -> C.CDLL:
         l.qa_workspace_bytes.restype = C.c_size_t
         l.qa_ground_state_open.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp, vp, vp,
                                            C.c_size_t, vp]
+        l.qa_ground_state_open_static.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp, vp, vp]
+        l.qa_static_workspace_bytes.restype = C.c_size_t
+        l.qa_static_workspace_last_error.restype = C.c_char_p
         l.qa_ground_state_closed.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp, vp,
                                              vp, C.c_size_t, vp]
         l.qa_ground_state_host.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, vp, vp, vp,
@@ -226,6 +232,31 @@ class Model:
             res["Vsensor"] = Vs
         if st is not None:
             res["stats"] = st
+        return res
+
+    def ground_state_static(self, Vg: torch.Tensor, algorithm="default", t=1.0, n_max=0, out=None, stream=None):
+        """qa_ground_state_open_static: the open-array search with the library's own static 16 MiB device workspace -- the C
+        call allocates nothing (for callers that cannot call cudaMalloc; limit: qa_workspace_bytes(P) <= 16 MiB, calls that
+        overlap on the GPU race on the array).  With `out` = dict(N, E) given, this binding allocates nothing either;
+        otherwise N and E are torch tensors it creates.  Returns dict(N, E)."""
+        if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
+            raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        self._check_device(Vg)
+        Vg = Vg.contiguous().view(-1, self.n_gate)
+        P, dev = Vg.shape[0], Vg.device
+        out = out or {}
+        N = out.get("N") if out.get("N") is not None else torch.empty((P, self.n_dot), dtype=torch.int32, device=dev)
+        E = out.get("E") if out.get("E") is not None else torch.empty(P, dtype=torch.float64, device=dev)
+        Vs = torch.empty((P, self.n_sensor), dtype=torch.float64, device=dev) if self.n_sensor else None
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        alg = ALG[algorithm] if isinstance(algorithm, str) else int(algorithm)
+        with torch.cuda.device(dev):
+            rc = lib().qa_ground_state_open_static(self._h, _ptr(Vg), P, alg, float(t), int(n_max), _ptr(N), _ptr(E), None,
+                                                   _ptr(Vs), None, C.c_void_p(s.cuda_stream))
+        _check(rc, "qa_ground_state_open_static")
+        res = {"N": N, "E": E}
+        if Vs is not None:
+            res["Vsensor"] = Vs
         return res
 
     def _call_ground_state(self, regime, Vg, P, N_hat, alg, t, n_max, N, E, xc, Vs, st, ws, sp):

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libqarray_b200.so")
 OBJ = os.path.join(HERE, "build")
-SOURCES = ["qa_api.cu", "qa_kernels_generic.cu", "qa_kernels_walk.cu", "qa_kernels_minplus.cu", "qa_kernels_fused.cu", "qa_kernels_fused_open.cu", "qa_kernels_thermal.cu", "qa_kernels_closed.cu", "qa_kernels_sensor.cu", "qa_kernels_thermal_sp.cu", "qa_kernels_minplus32.cu", "qa_kernels_fused_mid.cu"]
+SOURCES = ["qa_api.cu", "qa_kernels_generic.cu", "qa_kernels_walk.cu", "qa_kernels_minplus.cu", "qa_kernels_fused.cu", "qa_kernels_fused_open.cu", "qa_kernels_thermal.cu", "qa_kernels_closed.cu", "qa_kernels_sensor.cu", "qa_kernels_thermal_sp.cu", "qa_kernels_minplus32.cu", "qa_kernels_fused_mid.cu", "qa_static_workspace.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "--fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fvisibility=hidden", "-Xptxas", "-v"]
 

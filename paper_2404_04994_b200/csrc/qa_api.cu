@@ -790,6 +790,7 @@ const char *qa_status_string(qa_status s)
         case QA_ERR_OVERFLOW: return "brute force: (n_max+1)^n_dot >= 2^62";
         case QA_ERR_CUDA: return "CUDA error";
         case QA_ERR_UNSUPPORTED: return "unsupported (reserved; not returned by this version)";
+        case QA_ERR_STATIC_WORKSPACE: return "sweep too large for the static workspace (qa_static_workspace_last_error)";
     }
     return "unknown status";
 }
