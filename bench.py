@@ -376,9 +376,15 @@ def run_config5(args, rank, world, local_rank, steps=None, emit=True):
     px_step = B * P * len(algs)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
+    multi_spec = [("default", None), ("thresholded", 0.2), ("thresholded", 0.5)]
+    multi_out = [outs[a] for a, _ in algs]
+
     def step():
         for a, kw in algs:
             batch.ground_state(Vg, out=outs[a], **kw)
+
+    def step_multi():   # qa_ground_state_batch_multi: the three algorithms in one launch (V_g, N_c and the QP once per pixel)
+        batch.ground_state_multi(Vg, multi_spec, out=multi_out)
 
     def barrier():
         if world > 1:
@@ -407,6 +413,17 @@ def run_config5(args, rank, world, local_rank, steps=None, emit=True):
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         tot_ms = float(tt.item())
     ms_per_step = tot_ms / steps
+    # the same work through qa_ground_state_batch_multi (one launch for the three algorithms), for comparison
+    for _ in range(3):
+        step_multi()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for k in range(steps):
+        flush.fill_(k & 0xff)
+        evs[k][0].record()
+        step_multi()
+        evs[k][1].record()
+    torch.cuda.synchronize()
+    ms_multi = float(np.mean([a.elapsed_time(b) for a, b in evs]))
     if rank != 0:
         return None
     agree = {}
@@ -432,7 +449,11 @@ def run_config5(args, rank, world, local_rank, steps=None, emit=True):
                        "pixels_per_step_per_gpu": px_step, "l2": "flushed (256 MiB write) between timed steps",
                        "parallelism": f"array-range x{world}"},
             "agreement_with_default": agree,
-            "roofline": {"bound": "hbm", "kernel": "qa_fused_small_kernel (whole step: 3 launches)",
+            "one_launch": {"ms_per_step": ms_multi, "pixels_per_s": world * px_step / (ms_multi * 1e-3),
+                           "api": "qa_ground_state_batch_multi: the three algorithms in ONE launch (V_g, N_c and the QP once per "
+                                  "pixel; results bit-identical; 17 % fewer instructions, but measured slower on B200: DESIGN.md 5.5)",
+                           "algorithmic_bytes_per_step": B * P * (8 * g + len(algs) * (4 * n + 8))},
+            "roofline": {"bound": "hbm", "kernel": "qa_fused_open_kernel (whole step: 3 launches)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                          "bytes_per_pixel": bytes_px, "algorithmic_bytes_per_step": px_step * bytes_px,
                          "traffic_source": "not measured by this run; ncu figure in profiles/r02_config5_ncu.md",

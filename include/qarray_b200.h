@@ -241,6 +241,18 @@ QA_API qa_status qa_ground_state_batch(const qa_batch *batch, const double *d_Vg
                                        qa_algorithm alg, double t, int n_max, int32_t *d_N, double *d_E, double *d_xcont,
                                        qa_stats *d_stats, void *cuda_stream);
 
+/* Several algorithms on the SAME sweep in one launch: a dataset run searches every diagram with the default algorithm and
+ * with one or more thresholds (datasets for training; section IV.A: thresholds trade accuracy for speed).
+ * Semantically a loop over qa_ground_state_batch(batch, d_Vg, P, open, algs[a], ts[a]) -> d_N[a], d_E[a] for a = 0 ..
+ * n_alg - 1, with bit-identical results; V_g is read once and N_c and the continuous minimum (S1-S3, the QP) are computed
+ * once per pixel instead of once per algorithm.  Open arrays only; algs[a] is QA_ALG_DEFAULT or QA_ALG_THRESHOLDED (ts[a]
+ * in [0, 1], ignored for the default algorithm); 1 <= n_alg <= 4.  algs, ts, d_N, d_E: HOST arrays of n_alg entries, d_N[a] /
+ * d_E[a] device buffers shaped as in qa_ground_state_batch; d_xcont device or NULL (the same for every algorithm);
+ * d_stats device or NULL (summed over the algorithms).  Asynchronous on cuda_stream; needs no workspace; never allocates. */
+QA_API qa_status qa_ground_state_batch_multi(const qa_batch *batch, const double *d_Vg, int64_t P, int n_alg,
+                                             const qa_algorithm *algs, const double *ts, int32_t *const *d_N,
+                                             double *const *d_E, double *d_xcont, qa_stats *d_stats, void *cuda_stream);
+
 /* ---- diagnostics ------------------------------------------------------------------------------------------------- */
 /* (Measurement and cross-check aids -- FP64 issue-rate probe, per-kernel event timing, launch plan, kernel selection --
  * are declared in qarray_b200_aids.h; they are not part of the product surface.) */

@@ -27,7 +27,8 @@ EXPORTS = ["qa_model_create", "qa_model_set_sensor_dots", "qa_model_destroy", "q
            "qa_ground_state_batch", "qa_thermal_open", "qa_thermal_closed", "qa_sensor_response",
            "qa_sensor_response_workspace_bytes", "qa_last_launch_plan",
            "qa_last_launch_count", "qa_status_string", "qa_last_cuda_error", "qa_version", "qa_static_workspace_bytes",
-           "qa_static_workspace_init", "qa_static_workspace_last_error", "qa_ground_state_open_static"]
+           "qa_static_workspace_init", "qa_static_workspace_last_error", "qa_ground_state_open_static",
+           "qa_ground_state_batch_multi"]
 
 
 class qa_stats(C.Structure):
@@ -100,6 +101,7 @@ def lib() -> C.CDLL:
         l.qa_batch_destroy.argtypes = [vp]
         l.qa_batch_size.argtypes = [vp]
         l.qa_ground_state_batch.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, ip, dp, dp, vp, vp]
+        l.qa_ground_state_batch_multi.argtypes = [vp, dp, C.c_int64, C.c_int, vp, vp, vp, vp, dp, vp, vp]
         l.qa_thermal_open.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp, vp, vp, C.c_size_t, vp]
         l.qa_thermal_closed.argtypes = [vp, dp, C.c_int64, C.c_int, C.c_int, C.c_double, C.c_int, C.c_double, dp, dp, vp, vp,
                                         C.c_size_t, vp]
@@ -380,6 +382,47 @@ class Batch:
             res["xcont"] = xc
         if st is not None:
             res["stats"] = st
+        return res
+
+    def ground_state_multi(self, Vg: torch.Tensor, algorithms, want_xcont=False, want_stats=False, out=None, stream=None):
+        """qa_ground_state_batch_multi: several algorithms on the same sweep in one launch (V_g read once, N_c and the QP
+        once per pixel).  algorithms: list of ("default", None) / ("thresholded", t) pairs (or the strings "default" /
+        floats t).  out: optional list of dict(N, E), one per algorithm.  Returns a list of dict(N[B,P,n], E[B,P]) (the
+        first one also carries xcont / stats when asked for)."""
+        if not (isinstance(Vg, torch.Tensor) and Vg.is_cuda and Vg.dtype == torch.float64):
+            raise TypeError("Vg must be a CUDA float64 tensor (there is no CPU path)")
+        if Vg.device != self.device:
+            raise ValueError(f"Vg is on {Vg.device}, the batch lives on {self.device}")
+        B = len(self)
+        Vg = Vg.contiguous().view(B, -1, self.n_gate)
+        P, dev = Vg.shape[1], Vg.device
+        spec = []
+        for a in algorithms:
+            if isinstance(a, str):
+                a = (a, None)
+            elif isinstance(a, (int, float)):
+                a = ("thresholded", float(a))
+            spec.append((ALG[a[0]], 1.0 if a[1] is None else float(a[1])))
+        n_alg = len(spec)
+        res = []
+        for k in range(n_alg):
+            o = (out[k] if out is not None else None) or {}
+            N = o.get("N") if o.get("N") is not None else torch.empty((B, P, self.n_dot), dtype=torch.int32, device=dev)
+            E = o.get("E") if o.get("E") is not None else torch.empty((B, P), dtype=torch.float64, device=dev)
+            res.append({"N": N, "E": E})
+        xc = torch.empty((B, P, self.n_dot), dtype=torch.float64, device=dev) if want_xcont else None
+        st = torch.zeros(8, dtype=torch.int64, device=dev) if want_stats else None
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        algs = (C.c_int * n_alg)(*[a for a, _ in spec])
+        ts = (C.c_double * n_alg)(*[t for _, t in spec])
+        pN = (C.c_void_p * n_alg)(*[r["N"].data_ptr() for r in res])
+        pE = (C.c_void_p * n_alg)(*[r["E"].data_ptr() for r in res])
+        _check(lib().qa_ground_state_batch_multi(self._h, _ptr(Vg), P, n_alg, algs, ts, pN, pE, _ptr(xc), _ptr(st),
+                                                 C.c_void_p(s.cuda_stream)), "qa_ground_state_batch_multi")
+        if xc is not None:
+            res[0]["xcont"] = xc
+        if st is not None:
+            res[0]["stats"] = st
         return res
 
 

@@ -706,6 +706,32 @@ qa_status qa_ground_state_batch(const qa_batch *bt, const double *d_Vg, int64_t 
     return QA_OK;
 }
 
+qa_status qa_ground_state_batch_multi(const qa_batch *bt, const double *d_Vg, int64_t P, int n_alg, const qa_algorithm *algs,
+                                      const double *ts, int32_t *const *d_N, double *const *d_E, double *d_xcont,
+                                      qa_stats *d_stats, void *cuda_stream)
+{
+    qa_plan_reset();
+    if (!bt || P < 0 || n_alg < 1 || n_alg > QA_MULTI_MAX || !algs || !ts || !d_N || !d_E) return QA_ERR_INVALID_ARG;
+    if (P > 0 && !d_Vg) return QA_ERR_INVALID_ARG;
+    if (P > 0 && !on_device(bt->device)) return QA_ERR_INVALID_ARG;
+    QaMultiArgs ma{};
+    ma.n_alg = n_alg;
+    for (int a = 0; a < n_alg; ++a) {
+        if (algs[a] != QA_ALG_DEFAULT && algs[a] != QA_ALG_THRESHOLDED) return QA_ERR_INVALID_ARG;
+        if (algs[a] == QA_ALG_THRESHOLDED && !(ts[a] >= 0.0 && ts[a] <= 1.0)) return QA_ERR_INVALID_ARG;
+        if (P > 0 && (!d_N[a] || !d_E[a])) return QA_ERR_INVALID_ARG;
+        ma.thr[a] = algs[a] == QA_ALG_THRESHOLDED ? 1 : 0;
+        ma.t[a] = algs[a] == QA_ALG_THRESHOLDED ? ts[a] : 1.0;
+        ma.N[a] = d_N[a];
+        ma.E[a] = d_E[a];
+    }
+    if (P == 0) return QA_OK;
+    if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
+    QA_CUDA(qa_launch_fused_open_multi(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, bt->general, ma, d_xcont, d_stats,
+                                       static_cast<cudaStream_t>(cuda_stream)));
+    return QA_OK;
+}
+
 int qa_batch_size(const qa_batch *bt) { return bt ? bt->n_models : 0; }
 
 qa_status qa_measure_fp64_rate(double seconds, double *thread_inst_per_s, void *cuda_stream)

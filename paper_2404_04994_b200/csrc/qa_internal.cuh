@@ -67,6 +67,16 @@ struct QaCallArgs {
     int general_qp;  // c_dd has a positive off-diagonal: the QP continues with the primal active-set phase (R3)
 };
 
+// Several algorithms on one sweep in one launch (qa_ground_state_batch_multi): per pass the threshold and the outputs.
+constexpr int QA_MULTI_MAX = 4;
+struct QaMultiArgs {
+    int n_alg;
+    int thr[QA_MULTI_MAX];      // 1: thresholded (Eq. (9)), 0: default
+    double t[QA_MULTI_MAX];
+    int32_t *N[QA_MULTI_MAX];   // device [n_models * P * n]
+    double *E[QA_MULTI_MAX];    // device [n_models * P]
+};
+
 // Pair-energy table of the low QA_WALK_NL bits for the static walk: QL[b] = sum_{j<j', both set in b} M[a_j][a_j'],
 // a_j = n-1-j the dot of low bit j.  Passed by value (constant bank) so the unrolled walk reads it with static offsets.
 struct QaWalkTable {
@@ -105,6 +115,9 @@ cudaError_t qa_launch_fused_small(const QaDevModel *const *d_models, int n_model
 cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models, int n, int g, const double *d_Vg,
                                  int64_t P, QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
                                  qa_stats *d_stats, cudaStream_t stream);
+cudaError_t qa_launch_fused_open_multi(const QaDevModel *const *d_models, int n_models, int n, int g, const double *d_Vg,
+                                       int64_t P, int general_qp, const QaMultiArgs &ma, double *d_xcont, qa_stats *d_stats,
+                                       cudaStream_t stream);
 cudaError_t qa_launch_thermal(const QaDevModel *d_model, int n, QaWorkspace ws, QaCallArgs args, double kT,
                               double expect_cand, double *d_Nmean, double *d_Emin, qa_stats *d_stats, cudaStream_t stream);
 cudaError_t qa_launch_thermal_sp(const QaDevModel *d_model, int n, const double *QLhost, QaWorkspace ws, double kT,

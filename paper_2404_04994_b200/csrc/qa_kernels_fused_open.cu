@@ -39,6 +39,7 @@ constexpr int FO_THREADS = 128;
 // CTAs per SM the min-plus default walk is compiled for: 80 registers instead of 64, so that the table reads of several
 // batches are in flight before their DADDs (measured, config 5 default pass: 0.412 -> 0.399 ms)
 constexpr int FO_MP_CTAS = 6;
+constexpr int FO_MULTI_CTAS = 6;
 constexpr int FO_PX_RUN = 1;  // pixels per thread the launcher instantiates (measured, config 5: 1.21 ms per step vs 1.49 with 2)
 // PX = pixels per thread (2: every uniform operand serves two FMAs; 1: half the registers and shared memory per CTA, twice
 // the CTAs per SM -- the thresholded kernels are bound by latency, not by the FP64 pipe), PIX = FO_THREADS * PX per CTA
@@ -656,6 +657,358 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Several algorithms on the SAME sweep in one launch (qa_ground_state_batch_multi: a dataset run searches every diagram with
+// the default algorithm and with one or more thresholds, PAPER.md L500 / BASELINE.json configs[4]).  V_g is read once, the
+// model tables are staged once, N_c (S1) and the continuous minimum x (S2-S3, the QP) are computed once per pixel; S4-S7 then
+// run once per algorithm on the same x, with exactly the arithmetic of qa_fused_open_kernel (same order: the results are
+// bit-identical to separate calls, tests).  One pixel per thread; THR is a run-time, CTA-uniform switch per pass.
+template <int N, bool MP>
+__global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi_kernel(const QaDevModel *const *__restrict__ models,
+                                                                            const double *__restrict__ Vg, int64_t P, int g,
+                                                                            int general_qp, QaMultiArgs ma,
+                                                                            double *__restrict__ xcont, qa_stats *stats)
+{
+    constexpr int PIX = FO_THREADS;
+    __shared__ __align__(16) FoSmem<N, true, PIX> sm;
+    __shared__ double sx[N][PIX];  // the continuous minimum x of every pixel slot, read again by every pass
+    const int tid = threadIdx.x;
+    const int64_t p = (int64_t)blockIdx.x * PIX + tid;
+    const bool live = p < P;
+    const int64_t gp = (int64_t)blockIdx.y * P + (live ? p : P - 1);
+    const double *vp = Vg + gp * g;
+    const bool vec = (g & 1) == 0 && (reinterpret_cast<uintptr_t>(Vg) & 15u) == 0;
+    auto load_chunk = [&](int k0, double (&a)[8]) {
+        if (vec) {
+#pragma unroll
+            for (int k = 0; k < 8; k += 2) {
+                double2 ta = make_double2(0.0, 0.0);
+                if (k0 + k < g) ta = __ldg(reinterpret_cast<const double2 *>(vp + k0 + k));
+                a[k] = ta.x, a[k + 1] = ta.y;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = k0 + k < g ? __ldg(vp + k0 + k) : 0.0;
+        }
+    };
+    double va[8];
+    load_chunk(0, va);
+    const QaDevModel *__restrict__ mdl = models[blockIdx.y];
+    for (int e = tid; e < N * N; e += FO_THREADS) {
+        sm.MT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
+        sm.C[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
+    }
+    for (int e = tid; e < N * g; e += FO_THREADS) sm.CgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
+    for (int k = tid; k < (1 << N); k += FO_THREADS) sm.T[k] = mdl->QL[k];
+    const double EC = MP ? mdl->EC : 0.0;
+    __syncthreads();
+
+    // ---- S1-S3, once per pixel
+    double x[N];
+    {
+        double nc[N];
+#pragma unroll
+        for (int i = 0; i < N; ++i) nc[i] = 0.0;
+        for (int k0 = 0; k0 < g; k0 += 8) {
+            if (k0 > 0) load_chunk(k0, va);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (k0 + k < g) {
+#pragma unroll
+                    for (int i = 0; i < N; ++i) nc[i] = fma(sm.CgT[(k0 + k) * N + i], va[k], nc[i]);
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            x[i] = nc[i];
+            sm.nc[i][tid] = nc[i];
+        }
+    }
+    bool neg = false;
+#pragma unroll
+    for (int i = 0; i < N; ++i) neg |= x[i] < 0.0;
+    int rounds0 = 0;
+    bool failed0 = false, slowf = false;
+    if (neg) {
+        double nc[N];
+#pragma unroll
+        for (int i = 0; i < N; ++i) nc[i] = x[i];
+        rounds0 = fo_qp_open<N>(sm.C, nc, general_qp, x, failed0, slowf);
+    }
+    if (xcont && live && !slowf) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) xcont[gp * N + i] = x[i];
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) sx[i][tid] = x[i];
+    __syncthreads();  // every warp is done with C_gd: its storage becomes the sort's (thresholded passes)
+
+#pragma unroll 1
+    for (int a = 0; a < ma.n_alg; ++a) {
+        const bool thr = ma.thr[a] != 0;
+        const double tt = ma.t[a];
+        int32_t *__restrict__ outN = ma.N[a];
+        double *__restrict__ outE = ma.E[a];
+        // ---- S4 (Eq. (9), readings R4 / R10) and the base-point gradient
+        double hp[N];
+        unsigned fm = 0;
+        {
+            double d0[N], grad[N];
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                int32_t cn, bs;
+                qa_floor_ceil(sx[i][tid], tt, thr, bs, cn);
+                if (cn == 2) fm |= 1u << (N - 1 - i);
+                d0[i] = (double)bs - sm.nc[i][tid];
+                sm.base[i][tid] = bs;
+                grad[i] = 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < N; ++j) {
+#pragma unroll
+                for (int i = 0; i < N; ++i) grad[i] = fma(sm.MT[j * N + i], d0[j], grad[i]);
+            }
+#pragma unroll
+            for (int b = 0; b < N; ++b) hp[b] = grad[N - 1 - b] + 0.5 * sm.MT[(N - 1 - b) * N + (N - 1 - b)];
+        }
+        unsigned win = 0;
+        asm volatile("" ::: "memory");
+        if (!thr) {
+            if constexpr (MP) {
+                // min-plus split inside the thread (see qa_fused_open_kernel): pass 1 lower bounds per row of 16, pass 2 exact
+                constexpr int NW = 4, NU = N - NW, R = 1 << NU, GS = R < 4 ? R : 4, NG = R / GS;
+                double B[1 << NW], hu[NU];
+                double offw = EC, offu = EC;
+#pragma unroll
+                for (int j = 0; j < NW; ++j) offw += fabs(hp[j]);
+#pragma unroll
+                for (int j = 0; j < NU; ++j) {
+                    hu[j] = hp[NW + j];
+                    offu += fabs(hu[j]);
+                }
+                B[0] = offw;
+#pragma unroll
+                for (int w = 1; w < (1 << NW); ++w) B[w] = B[w & (w - 1)] + hp[fo_ctz(w)];
+                const double lo3 = NU >= 2 ? hu[NU >= 2 ? 1 : 0] + hu[0] : 0.0;
+                auto row_a = [&](int i, int ul) -> double {
+                    double ah = offu;
+#pragma unroll
+                    for (int j = NU - 1; j >= 2; --j)
+                        if ((i >> (j - 2)) & 1) ah += hu[j];
+                    if (NU >= 2) return ul == 0 ? ah : (ul == 1 ? ah + hu[0] : (ul == 2 ? ah + hu[NU >= 2 ? 1 : 0] : ah + lo3));
+                    return ul == 0 ? ah : ah + hu[0];
+                };
+                unsigned Lg[NG], rowmask = 0;
+#pragma unroll
+                for (int k = 0; k < NG; ++k) Lg[k] = 0xffffffffu;
+#pragma unroll 1
+                for (int i = 0; i < NG; ++i) {
+                    const double2 *__restrict__ T2 = reinterpret_cast<const double2 *>(sm.T + ((i * GS) << NW));
+                    unsigned l[GS];
+#pragma unroll
+                    for (int ul = 0; ul < GS; ++ul) {
+                        unsigned m0 = 0xffffffffu, m1 = 0xffffffffu;
+#pragma unroll
+                        for (int w = 0; w < (1 << NW); w += 4) {
+                            const double2 ta = T2[((ul << NW) | w) >> 1], tb = T2[((ul << NW) | (w + 2)) >> 1];
+                            const double y0 = B[w] + ta.x, y1 = B[w + 1] + ta.y, y2 = B[w + 2] + tb.x, y3 = B[w + 3] + tb.y;
+                            m0 = min(m0, min((unsigned)__double2hiint(y0), (unsigned)__double2hiint(y1)));
+                            m1 = min(m1, min((unsigned)__double2hiint(y2), (unsigned)__double2hiint(y3)));
+                        }
+                        const double lb = row_a(i, ul) + __hiloint2double((int)min(m0, m1), 0);
+                        l[ul] = (unsigned)__double2hiint(lb);
+                    }
+                    unsigned gmin = l[0];
+#pragma unroll
+                    for (int ul = 1; ul < GS; ++ul) gmin = min(gmin, l[ul]);
+                    unsigned nib = 0;
+#pragma unroll
+                    for (int ul = 0; ul < GS; ++ul) nib |= (l[ul] <= gmin + 2u ? 1u : 0u) << ul;
+                    rowmask |= nib << (i * GS);
+#pragma unroll
+                    for (int k = 0; k < NG; ++k)
+                        if (k == i) Lg[k] = gmin;
+                }
+                unsigned Lmin = Lg[0];
+#pragma unroll
+                for (int k = 1; k < NG; ++k) Lmin = min(Lmin, Lg[k]);
+                unsigned cand = 0;
+#pragma unroll
+                for (int k = 0; k < NG; ++k)
+                    if (Lg[k] <= Lmin + 2u) cand |= rowmask & (((1u << GS) - 1u) << (k * GS));
+                double best = __longlong_as_double(0x7ff0000000000000ll);
+                unsigned bkey = 0;
+                while (cand) {
+                    const int u = __ffs(cand) - 1;
+                    cand &= cand - 1u;
+                    const double av = row_a(u / GS, u % GS);
+                    const double *__restrict__ T = sm.T + (u << NW);
+#pragma unroll
+                    for (int w = 0; w < (1 << NW); ++w) {
+                        const double e = av + (B[w] + T[w]);
+                        if (e < best) {
+                            best = e;
+                            bkey = ((unsigned)u << NW) | (unsigned)w;
+                        }
+                    }
+                }
+                win = bkey;
+            } else {
+                // counting-order walk over all 2^N patterns (qa_fused_open_kernel, plain form)
+                constexpr int LB = N < 4 ? N : 4;
+                constexpr int NHI = N - LB;
+                double cl[LB], ch[NHI > 0 ? NHI : 1];
+                {
+                    double pre = 0.0;
+#pragma unroll
+                    for (int j = 0; j < N; ++j) {
+                        if (j < LB)
+                            cl[j] = hp[j] - pre;
+                        else
+                            ch[j - LB] = hp[j] - pre;
+                        pre += hp[j];
+                    }
+                }
+                double sl = 0.0, m = 0.0;
+#pragma unroll 1
+                for (int i = 0; i < (1 << NHI); ++i) {
+                    const double *__restrict__ T = sm.T + (i << LB);
+                    const unsigned kb = (unsigned)i << LB;
+                    if (i > 0) {
+                        double c = ch[NHI > 0 ? NHI - 1 : 0];
+#pragma unroll
+                        for (int j = NHI - 2; j >= 0; --j)
+                            if ((i >> j) & 1) c = ch[j];
+                        sl += c;
+                        const double e = sl + T[0];
+                        if (e < m) {
+                            m = e;
+                            win = kb;
+                        }
+                    }
+#pragma unroll
+                    for (int w = 1; w < (1 << LB); ++w) {
+                        sl += cl[fo_ctz(w)];
+                        const double e = sl + T[w];
+                        if (e < m) {
+                            m = e;
+                            win = kb + w;
+                        }
+                    }
+                }
+            }
+        } else {
+            // thresholded: compaction of the free dots, bucket sort of the CTA's pixels by k, walk, hand back
+            if (tid < 16) sm.bucket[tid] = 0;
+            __syncthreads();
+            {
+                double pre = 0.0;
+                int jj = 0;
+                unsigned low = 0;
+                unsigned long long xm = 0;
+#pragma unroll
+                for (int b = 0; b < N; ++b) {
+                    if ((fm >> b) & 1u) {
+                        sm.cs[jj][tid] = hp[b] - pre;
+                        pre += hp[b];
+                        xm |= (unsigned long long)((1u << b) | low) << (8 * jj);
+                        low |= 1u << b;
+                        ++jj;
+                    }
+                }
+                const int kf = live ? jj : 0;
+                sm.sort.xm[tid] = xm;
+                sm.sort.kfree[tid] = (unsigned char)kf;
+                sm.sort.wkey[tid] = 0;
+                const int rk = fo_bucket_rank(sm.bucket, N - kf);
+                __syncthreads();
+                int start = 0;
+#pragma unroll
+                for (int bkt = 0; bkt <= N; ++bkt)
+                    if (bkt < N - kf) start += sm.bucket[bkt];
+                sm.sort.order[start + rk] = (unsigned short)tid;
+            }
+            __syncthreads();
+            {
+                const int slot = sm.sort.order[tid];
+                const unsigned nst = 1u << sm.sort.kfree[slot];
+                const unsigned long long xm = sm.sort.xm[slot];
+                double sl = 0.0, best = 0.0;
+                unsigned key = 0, bkey = 0;
+                for (unsigned st = 1; st < nst; ++st) {
+                    const int j = __ffs(st) - 1;
+                    sl += sm.cs[j][slot];
+                    key ^= (unsigned)(xm >> (8 * j)) & 0xffu;
+                    const double e = sl + sm.T[key];
+                    if (e < best) {
+                        best = e;
+                        bkey = key;
+                    }
+                }
+                sm.sort.wkey[slot] = (unsigned char)bkey;
+            }
+            __syncthreads();
+            win = sm.sort.wkey[tid];
+        }
+        // (compiler barriers: without them the M values the gradient phase loaded are kept for the epilogue, in local memory)
+        asm volatile("" ::: "memory");
+        // ---- S7: N* = base + bits of the winner; E(N*) = 1/2 d^T M d from the definition (Eq. (C1))
+        {
+            int32_t Ns[N];
+            double d[N], row[N];
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                Ns[i] = sm.base[i][tid] + (int32_t)((win >> (N - 1 - i)) & 1u);
+                d[i] = (double)Ns[i] - sm.nc[i][tid];
+                row[i] = 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < N; ++j) {
+#pragma unroll
+                for (int i = 0; i < N; ++i) row[i] = fma(sm.MT[j * N + i], d[j], row[i]);
+            }
+            double Ed = 0.0;
+#pragma unroll
+            for (int i = 0; i < N; ++i) Ed = fma(d[i], row[i], Ed);
+            if (live) {
+                outE[gp] = 0.5 * Ed;
+                if (N % 4 == 0 && (reinterpret_cast<uintptr_t>(outN) & 15u) == 0) {
+#pragma unroll
+                    for (int i = 0; i + 3 < N; i += 4)
+                        *reinterpret_cast<int4 *>(outN + gp * N + i) = make_int4(Ns[i], Ns[i + 1], Ns[i + 2], Ns[i + 3]);
+                } else {
+#pragma unroll
+                    for (int i = 0; i < N; ++i) outN[gp * N + i] = Ns[i];
+                }
+            }
+        }
+        asm volatile("" ::: "memory");
+        int rounds = rounds0, kfree = __popc(fm);
+        bool failed = failed0;
+        if (live && slowf) {  // deferred pixel (see fo_slow_pixel): redone from scratch with this pass's algorithm
+            int st3[3];
+            QaCallArgs sa{0, 0, thr ? (int)QA_ALG_THRESHOLDED : (int)QA_ALG_DEFAULT, tt, 0, general_qp};
+            if (thr)
+                fo_slow_pixel<N, true>(sm.MT, sm.C, sm.T, mdl, Vg, gp, sa, outN, outE, xcont, nullptr, st3);
+            else
+                fo_slow_pixel<N, false>(sm.MT, sm.C, sm.T, mdl, Vg, gp, sa, outN, outE, xcont, nullptr, st3);
+            rounds = st3[0];
+            failed = st3[1] != 0;
+            kfree = st3[2];
+        }
+        if (stats) {
+            qa_warp_count(&stats->n_pixels, live ? 1 : 0);
+            qa_warp_count(&stats->n_qp_pixels, (live && neg) ? 1 : 0);
+            qa_warp_count(&stats->n_qp_rounds, live ? rounds : 0);
+            qa_warp_count(&stats->n_qp_failed, (live && failed) ? 1 : 0);
+            const int64_t ne = live ? (int64_t)1 << kfree : 0;
+            qa_warp_count(&stats->n_candidates_enumerated, ne);
+            qa_warp_count(&stats->n_candidates_scored, ne);
+        }
+    }
+}
+
 template <int N>
 cudaError_t launch_fused_open_n(const QaDevModel *const *d_models, int n_models, const double *d_Vg, int64_t P, int g,
                                 QaCallArgs args, int32_t *d_N, double *d_E, double *d_xcont, double *d_Vs,
@@ -698,4 +1051,36 @@ cudaError_t qa_launch_fused_open(const QaDevModel *const *d_models, int n_models
         default: return cudaErrorInvalidValue;
     }
 #undef CALL
+}
+
+// Open arrays, n <= QA_FUSED_MAXN, no sensor dots: ma.n_alg passes (default / thresholded) over one sweep in one launch.
+cudaError_t qa_launch_fused_open_multi(const QaDevModel *const *d_models, int n_models, int n, int g, const double *d_Vg,
+                                       int64_t P, int general_qp, const QaMultiArgs &ma, double *d_xcont, qa_stats *d_stats,
+                                       cudaStream_t stream)
+{
+    qa_plan_add("qa_fused_open_multi_kernel");
+    if (n_models > 65535 || ma.n_alg < 1 || ma.n_alg > QA_MULTI_MAX) return cudaErrorInvalidValue;
+    const dim3 grid((unsigned)((P + FO_THREADS - 1) / FO_THREADS), (unsigned)n_models);
+#define CALL(NN)                                                                                                         \
+    do {                                                                                                                 \
+        if (NN >= 5 && general_qp == 0)                                                                                  \
+            qa_fused_open_multi_kernel<NN, (NN >= 5)><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, general_qp, ma, \
+                                                                                    d_xcont, d_stats);                  \
+        else                                                                                                             \
+            qa_fused_open_multi_kernel<NN, false><<<grid, FO_THREADS, 0, stream>>>(d_models, d_Vg, P, g, general_qp, ma,  \
+                                                                                d_xcont, d_stats);                      \
+    } while (0)
+    switch (n) {
+        case 1: CALL(1); break;
+        case 2: CALL(2); break;
+        case 3: CALL(3); break;
+        case 4: CALL(4); break;
+        case 5: CALL(5); break;
+        case 6: CALL(6); break;
+        case 7: CALL(7); break;
+        case 8: CALL(8); break;
+        default: return cudaErrorInvalidValue;
+    }
+#undef CALL
+    return cudaGetLastError();
 }

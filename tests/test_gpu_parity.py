@@ -471,6 +471,55 @@ def test_batch_equals_loop_and_oracle(api):
     assert e.value.status == 4
 
 
+@pytest.mark.parametrize("n", [2, 4, 5, 7, 8])
+def test_batch_multi_equals_separate_calls(api, n):
+    """qa_ground_state_batch_multi (several algorithms on one sweep in one launch: S1-S3 once per pixel) is a loop over
+    qa_ground_state_batch: N, E, x bit-identical, statistics summed; ragged P; a pass order with the default algorithm in
+    the middle; QP pixels present (negative N_c)."""
+    B, P = 3, 333
+    wls = [wl.random_open(n, n + 1, P, seed=4000 + 10 * n + j, lo=-0.8, hi=2.6) for j in range(B)]
+    models = [api.Model(w.C_dd, w.C_gd) for w in wls]
+    batch = api.Batch(models)
+    Vg = torch.from_numpy(np.stack([w.Vg for w in wls])).cuda()
+    algs = [("thresholded", 0.2), ("default", None), ("thresholded", 0.5), ("thresholded", 0.0)]
+    rm = batch.ground_state_multi(Vg, algs, want_xcont=True, want_stats=True)
+    torch.cuda.synchronize()
+    assert api.last_launch_plan()[0] == ["qa_fused_open_multi_kernel"]
+    tot = {}
+    for k, (name, t) in enumerate(algs):
+        kw = dict(algorithm=name) if t is None else dict(algorithm=name, t=t)
+        r1 = batch.ground_state(Vg, want_xcont=True, want_stats=True, **kw)
+        assert torch.equal(rm[k]["N"], r1["N"]) and torch.equal(rm[k]["E"], r1["E"])
+        assert torch.equal(rm[0]["xcont"], r1["xcont"])
+        for key, v in api.stats_dict(r1["stats"]).items():
+            tot[key] = tot.get(key, 0) + v
+    assert api.stats_dict(rm[0]["stats"]) == tot and tot["n_qp_pixels"] > 0
+    # against the oracle, one member
+    om = oracle.Model(wls[1].C_dd, wls[1].C_gd)
+    for k, (name, t) in enumerate(algs):
+        okw = dict(algorithm=name) if t is None else dict(algorithm=name, t=t)
+        o = om.ground_state(wls[1].Vg, **okw)
+        compare(rm[k]["N"][1].cpu().numpy(), rm[k]["E"][1].cpu().numpy(), o, om.EC, gpu_x=rm[0]["xcont"][1].cpu().numpy())
+    with pytest.raises(api.QaError):
+        batch.ground_state_multi(Vg, [("brute", None)])
+    with pytest.raises(api.QaError):
+        batch.ground_state_multi(Vg, [0.2] * 5)
+
+
+def test_batch_multi_general_cdd(api):
+    """A c_dd with positive off-diagonals (every pixel takes the general QP solver's slow path) through the multi call."""
+    wls = [wl.random_general(6, 6, 97, seed=4200 + j) for j in range(2)] if hasattr(wl, "random_general") else None
+    if wls is None:
+        pytest.skip("no general-c_dd generator")
+    models = [api.Model(w.C_dd, w.C_gd) for w in wls]
+    batch = api.Batch(models)
+    Vg = torch.from_numpy(np.stack([w.Vg for w in wls])).cuda()
+    rm = batch.ground_state_multi(Vg, ["default", 0.3])
+    for k, kw in enumerate((dict(algorithm="default"), dict(algorithm="thresholded", t=0.3))):
+        r1 = batch.ground_state(Vg, **kw)
+        assert torch.equal(rm[k]["N"], r1["N"]) and torch.equal(rm[k]["E"], r1["E"])
+
+
 # ---- edge cases -----------------------------------------------------------------------------------------------------
 def test_edge_cases(api):
     w = wl.config1(4, 4)
