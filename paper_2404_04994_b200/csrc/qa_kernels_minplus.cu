@@ -19,7 +19,18 @@
 // (LDCU.64; measured: one indexed LDCU per ~4 cycles per scheduler), and every entry serves the PX = 2 pixels a thread
 // walks at once.  DESIGN.md section 6 lists what else was measured (register-bank conflicts of the min3, LDS vs LDCU).
 //
-//   qa_minplus_walk_kernel (pass 1; a lower bound per thread):
+//   Keys.  The pruned and the one-kernel variants compare the HIGH words as described below.  qa_minplus_walk_kernel itself
+//   (ENC = 1) uses fixed-point keys: a per-pixel constant C' = 1.5 * 2^(52-k) is folded into B[0] and into a0, so every
+//   B[w], y and A[u] lies in [2^(52-k), 2^(53-k)) and shares one exponent; the LOW 32 bits of the pattern are then the
+//   energy in units of 2^-k rounded to nearest (one rounding of <= 1/2 unit per addition), m_u = min_w lo32(y) and
+//   L_t = min_u (lo32(C' + A[u]) + m_u) are integer operations (VIMNMX3, VIADDMNMX), and k is chosen per pixel from a
+//   thread-independent bound of A + y (E(base), E_C, |h_j| of all dots, the sum of all pair energies) so that A + y < 2^31
+//   units: no wrap.  An estimate passes at most 10 roundings (B: C' + 4 subset adds, y: 1, A: C' + 3 adds, the sum: exact),
+//   so |L_t - min e_t| <= 5 units and the thread of the arg min (and of every tie) has L_t <= min L + 10; the kernel keeps
+//   the lanes within MP_ENC_SLACK = 16.  One unit is ~2^-30 of the bound (~4e-8 E_C on config 4; the high-word keys resolve
+//   2^-20 of the value), so pass 2 sees fewer survivors, and the row bound costs an integer add instead of a DADD.
+//   Measured: walk 87.4 -> 85.0 us, identical N and E on every test.
+//   qa_minplus_walk_kernel (pass 1; a lower bound per thread; the high-word form):
 //       m_u  = min_w hi32(y)                               (ALU pipe, VIMNMX3)
 //       LB_u = A[u] + double(m_u, 0)   <= min_w e(t,u,w)   (truncation and rounding are monotone)
 //       L_t  = min_u hi32(LB_u)
@@ -45,6 +56,7 @@ namespace {
 
 constexpr int MP_THREADS = 256;
 constexpr int MF_THREADS = 256;
+constexpr unsigned MP_ENC_SLACK = 16u;  // fixed-point keys: how far above the minimum a bound may lie (see the kernel)
 
 template <int NL>
 struct alignas(16) MpTable {
@@ -97,10 +109,34 @@ __device__ __forceinline__ void mp_lmin(unsigned &L, double lb)
     asm volatile("{ .reg .b32 lo, hi; mov.b64 {lo,hi}, %1; min.u32 %0, %0, hi; }" : "+r"(L) : "d"(lb));
 }
 
+// ---- fixed-point keys (ENC = 1): every y carries the pixel's constant C' = 1.5 * 2^(52 - k) (folded into B[w]), so all of
+// them share one exponent and the LOW 32 bits of the pattern are the energy in units of 2^-k, rounded to nearest.
+// m0 = min(m0, lo32(y[0..3])), m1 = min(m1, lo32(y[4..7]))
+__device__ __forceinline__ void mp_min8_lo(unsigned &m0, unsigned &m1, const double (&y)[8])
+{
+    asm volatile(
+        "{ .reg .b32 hi, l0, l1, l2, l3, l4, l5, l6, l7;\n"
+        " mov.b64 {l0,hi}, %2; mov.b64 {l1,hi}, %3; mov.b64 {l2,hi}, %4; mov.b64 {l3,hi}, %5;\n"
+        " mov.b64 {l4,hi}, %6; mov.b64 {l5,hi}, %7; mov.b64 {l6,hi}, %8; mov.b64 {l7,hi}, %9;\n"
+        " min.u32 l0, l0, l1; min.u32 %0, %0, l0; min.u32 l2, l2, l3; min.u32 %0, %0, l2;\n"
+        " min.u32 l4, l4, l5; min.u32 %1, %1, l4; min.u32 l6, l6, l7; min.u32 %1, %1, l6; }"
+        : "+r"(m0), "+r"(m1)
+        : "d"(y[0]), "d"(y[1]), "d"(y[2]), "d"(y[3]), "d"(y[4]), "d"(y[5]), "d"(y[6]), "d"(y[7]));
+}
+// L = min(L, alo + m): integer lower bound of a row (alo = lo32(C' + A[u]))
+__device__ __forceinline__ void mp_lmin_int(unsigned &L, unsigned alo, unsigned m)
+{
+    asm volatile("{ .reg .b32 s; add.u32 s, %1, %2; min.u32 %0, %0, s; }" : "+r"(L) : "r"(alo), "r"(m));
+}
+__device__ __forceinline__ unsigned mp_lo32(double x)
+{
+    return (unsigned)__double2loint(x);
+}
+
 // One chunk of the walk: the four u = 4 i + {0..3} against every w, for PX pixels, as a software pipeline over batches of
 // eight DADDs: batch g is issued, then the minima of batch g-1 are taken, then the lower bound of a u whose last batch
 // was g-2 is formed, then that of g-3 enters L.  q = the chunk's 4 * 2^NW table entries; a[ul][px] = A[4 i + ul].
-template <int NW, int PX>
+template <int NW, int PX, int ENC = 0>
 __device__ __forceinline__ void mp_chunk(const double2 *__restrict__ q, const double (&B)[PX][1 << NW],
                                          const double (&a)[4][PX], unsigned (&L)[PX])
 {
@@ -130,7 +166,24 @@ __device__ __forceinline__ void mp_chunk(const double2 *__restrict__ q, const do
             }
             mp_add8(y[g & 1], bb, qq);
         }
-        if (g >= 1 && g <= G) mp_min8(m[(g - 1) / BPU][0], m[(g - 1) / BPU][1], y[(g - 1) & 1]);
+        if (g >= 1 && g <= G) {
+            if (ENC)
+                mp_min8_lo(m[(g - 1) / BPU][0], m[(g - 1) / BPU][1], y[(g - 1) & 1]);
+            else
+                mp_min8(m[(g - 1) / BPU][0], m[(g - 1) / BPU][1], y[(g - 1) & 1]);
+        }
+        if (ENC) {  // a[ul][px] holds C' + A[u]: its low word plus the row minimum is the row's bound, in units of 2^-k
+            if (g >= 2 && g - 2 < G && (g - 2) % BPU == BPU - 1) {
+                const int ul = (g - 2) / BPU;
+                if (PX == 2) {
+                    mp_lmin_int(L[0], mp_lo32(a[ul][0]), m[ul][0]);
+                    mp_lmin_int(L[PX - 1], mp_lo32(a[ul][PX - 1]), m[ul][1]);
+                } else {
+                    mp_lmin_int(L[0], mp_lo32(a[ul][0]), min(m[ul][0], m[ul][1]));
+                }
+            }
+            continue;
+        }
         if (g >= 2 && g - 2 < G && (g - 2) % BPU == BPU - 1) {
             const int ul = (g - 2) / BPU;
             if (PX == 2) {
@@ -150,11 +203,12 @@ __device__ __forceinline__ void mp_chunk(const double2 *__restrict__ q, const do
 
 // ---------------------------------------------------------------------------------------------------------------------
 // pass 1.  PX pixels per thread at once: every table entry fetched into a uniform register serves PX DADDs.
-template <int NH, int NU, int NW, int PX, int MINB>
+template <int NH, int NU, int NW, int PX, int MINB, int ENC_ = 0>
 __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const QaDevModel *__restrict__ mdl,
                                                                            const __grid_constant__ MpTable<NU + NW> tab,
                                                                            QaWorkspace ws)
 {
+    constexpr int ENC = ENC_;
     constexpr int NL = NU + NW;
     constexpr int N = NL + NH;
     constexpr int TPP = 1 << NH;             // threads per pixel
@@ -176,6 +230,14 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
     for (int j = 0; j < NL; ++j) v[j] = mdl->VT[t * NL + j];
     const double EC = mdl->EC;
     const double QH = mdl->QHT[t];
+    // ENC: sum of ALL pair energies M_ij, i < j (>= the pair energy of any pattern: M >= 0) = pairs among the high bits +
+    // pairs among the low bits + every cross term
+    double QSUM = 0.0;
+    if (ENC) {
+        QSUM = (mdl->QHT[TPP - 1] - EC) + tab.q[(1 << NL) - 1];
+#pragma unroll
+        for (int j = 0; j < NL; ++j) QSUM += mdl->VT[(TPP - 1) * NL + j];
+    }
 
     // Every slot (the TPP threads of one pixel group) is an independent worker; consecutive workers sit in different
     // CTAs so that a ragged last round is spread over all SMs.
@@ -202,6 +264,7 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
         double B[PX][1 << NW];  // B[w]: bits of w added from the highest to the lowest
         double hu[PX][NU];      // h' of the u bits
         double a0[PX], lo3[PX];
+        double Cenc[PX];  // ENC: the pixel's fixed-point constant C' = 1.5 * 2^(52 - k)
 #pragma unroll
         for (int px = 0; px < PX; ++px) {
             const double myv = nextv[px];
@@ -220,15 +283,29 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
                     offu += fabs(hj);
                 }
             }
-            double be = mp_shfl(myv, N) + QH;
+            const double e0h = mp_shfl(myv, N);
+            double be = e0h + QH, sumhigh = 0.0;
 #pragma unroll
             for (int jh = 0; jh < NH; ++jh) {
                 const double hv = mp_shfl(myv, N - 1 - NL - jh);
                 if ((t >> jh) & 1u) be += hv;
+                if (ENC) sumhigh += fabs(hv);
             }
             a0[px] = be + offu;
             lo3[px] = hu[px][1] + hu[px][0];
             B[px][0] = offw;
+            if (ENC) {
+                // Thread-independent bound of A[u] + y over the whole pixel:  A <= E(base) + QSUM + E_C + sum_high |h| +
+                // 2 sum_u |h| + NU QSUM,  y <= E_C + 2 sum_w |h| + (NW + 1) QSUM.  bound < 2^(ex + 1); one unit = 2^(ex - 30),
+                // so that A + y < 2^31 units and the integer sums below cannot wrap.
+                const double bound = fabs(e0h) + 2.0 * ((offw + offu) + sumhigh) + (double)(NL + 2) * QSUM;
+                const int eb = (__double2hiint(bound) >> 20) & 0x7ff;   // biased exponent of the bound
+                Cenc[px] = __hiloint2double(((eb + 22) << 20) | 0x80000, 0);
+                a0[px] += Cenc[px];     // (every A[u] of the chunk loop then carries C': one rounding to the grid per add)
+                B[px][0] += Cenc[px];
+            } else {
+                Cenc[px] = 0.0;
+            }
 #pragma unroll
             for (int w = 1; w < (1 << NW); ++w) B[px][w] = B[px][w & (w - 1)] + hw[mp_ctz(w)];
         }
@@ -258,13 +335,13 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
                 a[2][px] = ah + hu[px][1];
                 a[3][px] = ah + lo3[px];
             }
-            mp_chunk<NW, PX>(q, B, a, L);
+            mp_chunk<NW, PX, ENC>(q, B, a, L);
         }
 
 #pragma unroll
         for (int px = 0; px < PX; ++px) {
             const unsigned wmin = __reduce_min_sync(0xffffffffu, L[px]);
-            const unsigned ball = __ballot_sync(0xffffffffu, L[px] <= wmin + 2u);
+            const unsigned ball = __ballot_sync(0xffffffffu, L[px] <= wmin + (ENC ? MP_ENC_SLACK : 2u));
             const int64_t p = grp * PX + px;
             if (lane == 0 && p < P) ws.rec[p * WPP + wq] = make_uint2(wmin, ball);
         }
@@ -869,7 +946,7 @@ cudaError_t launch_finish(const QaDevModel *d_model, QaWorkspace ws, int32_t *d_
                          d_E, slack);
 }
 
-template <int NH, int NU, int NW, int PX, int MINB>
+template <int NH, int NU, int NW, int PX, int MINB, int ENC = 0>
 cudaError_t launch_mp(const QaDevModel *d_model, const double *QLhost, QaWorkspace ws, int32_t *d_N, double *d_E,
                       int sm_count, cudaStream_t stream)
 {
@@ -878,19 +955,19 @@ cudaError_t launch_mp(const QaDevModel *d_model, const double *QLhost, QaWorkspa
     MpTable<NL> local;  // the first 2^NL entries of the model's table (the table of fewer low bits is a prefix)
     for (int b = 0; b < (1 << NL); ++b) local.q[b] = QLhost[b];
     int per_sm = 0;
-    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_walk_kernel<NH, NU, NW, PX, MINB>,
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qa_minplus_walk_kernel<NH, NU, NW, PX, MINB, ENC>,
                                                                     MP_THREADS, 0);
     if (err != cudaSuccess) return err;
     if (per_sm < 1) per_sm = 1;
     int64_t grid = (int64_t)sm_count * per_sm;
     const int64_t need = ((ws.P + PX - 1) / PX + SLOTS - 1) / SLOTS;
     if (grid > need) grid = need;
-    err = qa_launch_pdl(qa_minplus_walk_kernel<NH, NU, NW, PX, MINB>, dim3((unsigned)grid), dim3(MP_THREADS), stream, d_model,
+    err = qa_launch_pdl(qa_minplus_walk_kernel<NH, NU, NW, PX, MINB, ENC>, dim3((unsigned)grid), dim3(MP_THREADS), stream, d_model,
                         local, ws);
     if (err != cudaSuccess) return err;
     qa_plan_add("qa_minplus_finish_kernel");
     qa_timing_mark(stream);
-    return launch_finish<NH, NU, NW>(d_model, ws, d_N, d_E, sm_count, stream);
+    return launch_finish<NH, NU, NW>(d_model, ws, d_N, d_E, sm_count, stream, ENC ? MP_ENC_SLACK : 2u);
 }
 
 }  // namespace
@@ -930,7 +1007,9 @@ cudaError_t qa_launch_minplus_walk(const QaDevModel *d_model, int n, const doubl
         }
     }
     qa_plan_add("qa_minplus_walk_kernel");
-#define MP_CALL(NH) launch_mp<NH, 4, 4, 2, 2>(d_model, QLhost, ws, d_N, d_E, sm_count, stream)
+    // ENC = 1: fixed-point keys on the low words (see the kernel); the high-word keys (ENC = 0) remain in the pruned and the
+    // one-kernel variants
+#define MP_CALL(NH) launch_mp<NH, 4, 4, 2, 2, 1>(d_model, QLhost, ws, d_N, d_E, sm_count, stream)
     switch (n) {
         case 13: return MP_CALL(5);
         case 14: return MP_CALL(6);

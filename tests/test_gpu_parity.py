@@ -209,7 +209,9 @@ def test_minplus_walk_extreme_inputs(api):
     """Pixels far outside the operating range: every dot clamped (N_c << 0, huge positive h) and large occupations."""
     w = wl.config4(6, 5)
     rng = np.random.default_rng(7)
-    Vg = np.concatenate([w.Vg, -50.0 * np.abs(rng.standard_normal((7, 16))), w.Vg[:9] * 40.0, np.zeros((3, 16))])
+    # (the last two blocks stress the per-pixel fixed-point scale of the walk's keys: energies of 1e12 and of 1e-18 E_C)
+    Vg = np.concatenate([w.Vg, -50.0 * np.abs(rng.standard_normal((7, 16))), w.Vg[:9] * 40.0, np.zeros((3, 16)),
+                         w.Vg[:6] * 1.0e6, w.Vg[:6] * 1.0e-9])
     w.Vg, w.W, w.H = np.ascontiguousarray(Vg), Vg.shape[0], 1
     for variant in (0, 1, 2, 3, 4):
         check(api, w, variant=variant, algorithm="default")
