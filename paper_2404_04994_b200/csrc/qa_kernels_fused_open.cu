@@ -103,12 +103,12 @@ struct FoSort {  // thresholded: bookkeeping of the bucket sort and the walk
     unsigned char wkey[THR ? PIX : 1];     // winning pattern
 };
 
-template <int N, bool THR, int PIX>
+template <int N, bool THR, int PIX, bool KEEP_NC = false>
 struct FoSmem {
     double MT[N * N];          // MT[j*N + i] = M[i][j]: the N values a column step needs are contiguous
     double C[N * N];           // c_dd, row-major (QP)
     double T[1 << N];          // pair table of the bit patterns: T[b] = QL[b] (bit j <-> dot N-1-j)
-    double nc[N][PIX];      // N_c of every pixel slot, parked during the walk (registers: 4 CTAs per SM)
+    double nc[KEEP_NC ? N : 1][KEEP_NC ? PIX : 1];  // N_c of every pixel slot (multi-algorithm kernel: read by every pass)
     int32_t base[N][PIX];   // ... and the base point
     double cs[THR ? N : 1][PIX];     // thresholded: c_j of the compacted free dots, per pixel slot
     int bucket[16];                  // thresholded: pixels of the CTA per number of free dots (outside the union below:
@@ -297,6 +297,7 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
         }
     }
     double d0[FO_PX][N];
+    double Ebase[FO_PX], dE[FO_PX];  // E(base) and the winner's energy relative to it: E(N*) = E(base) + dE (see S7 below)
 #pragma unroll
     for (int px = 0; px < FO_PX; ++px) {
         // S2 + S3
@@ -321,8 +322,7 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
             qa_floor_ceil(x[i], args.t, THR, bs, cn);
             if (cn == 2) fm |= 1u << (N - 1 - i);
             d0[px][i] = (double)bs - nc[px][i];
-            // N_c and the base point wait in shared memory while the gradient and the walk have the registers
-            sm.nc[i][px * FO_THREADS + tid] = nc[px][i];
+            // the base point waits in shared memory while the gradient and the walk have the registers
             sm.base[i][px * FO_THREADS + tid] = bs;
         }
         freem[px] = fm;
@@ -351,6 +351,14 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
             const double hm = 0.5 * sm.MT[(N - 1 - b) * N + (N - 1 - b)];
 #pragma unroll
             for (int px = 0; px < FO_PX; ++px) hp[px][b] = grad[px][N - 1 - b] + hm;
+        }
+        // E(base) = 1/2 d0^T M d0 (Eq. (C1)) from the gradient that is already there
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            double eb = 0.0;
+#pragma unroll
+            for (int i = 0; i < N; ++i) eb = fma(d0[px][i], grad[px][i], eb);
+            Ebase[px] = 0.5 * eb;
         }
     }
 
@@ -450,6 +458,7 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
                 }
             }
             win[px] = bkey;
+            dE[px] = best - (offw + offu);  // (the offsets are exact sums of |h| and E_C: their rounding is that of best itself)
         }
     } else if constexpr (!THR) {
         // counting-order walk over all 2^N patterns, both pixels at once (qa_kernels_walk.cu).  A real loop over chunks of
@@ -507,6 +516,8 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
                 }
             }
         }
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) dE[px] = m[px];
     } else {
         // compaction of the free dots (ascending bit position), bucket sort of the CTA's pixels by k, walk, hand back
         __syncthreads();  // every warp is done with C_gd: its storage becomes the sort's
@@ -564,45 +575,30 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
                 }
             }
             sm.sort.wkey[slot] = (unsigned char)bkey;
+            sm.cs[0][slot] = best;  // (the slot's c_j are dead: this thread was their only reader)
         }
         __syncthreads();
 #pragma unroll
-        for (int px = 0; px < FO_PX; ++px) win[px] = sm.sort.wkey[px * FO_THREADS + tid];
+        for (int px = 0; px < FO_PX; ++px) {
+            win[px] = sm.sort.wkey[px * FO_THREADS + tid];
+            dE[px] = sm.cs[0][px * FO_THREADS + tid];
+        }
     }
 
     // (compiler barrier: without it the M values the gradient phase loaded are kept for the epilogue -- in local memory)
     asm volatile("" ::: "memory");
-    // ---- S7 (+ S8): N* = base + bits of the winner; E(N*) = 1/2 d^T M d from the definition (Eq. (C1))
+    // ---- S7 (+ S8): N* = base + bits of the winner.  E(N*) = E(base) + dE: E(base) from the definition (Eq. (C1)) and dE
+    // the increment the walk has minimised (Eq. (C1) expanded around the base point: dE = sum_{i in b} h_i + pairs(b)); the
+    // rounding of both is a few ulp of E_C-sized terms, far inside the 1e-9 max(|E|, E_C) of the parity tests
     int32_t Ns[FO_PX][N];
-    double d[FO_PX][N];
 #pragma unroll
     for (int px = 0; px < FO_PX; ++px)
 #pragma unroll
-        for (int i = 0; i < N; ++i) {
-            Ns[px][i] = sm.base[i][px * FO_THREADS + tid] + (int32_t)((win[px] >> (N - 1 - i)) & 1u);
-            d[px][i] = (double)Ns[px][i] - sm.nc[i][px * FO_THREADS + tid];
-        }
-    double row[FO_PX][N];
-#pragma unroll
-    for (int px = 0; px < FO_PX; ++px)
-#pragma unroll
-        for (int i = 0; i < N; ++i) row[px][i] = 0.0;
-#pragma unroll
-    for (int j = 0; j < N; ++j) {
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            const double mij = sm.MT[j * N + i];
-#pragma unroll
-            for (int px = 0; px < FO_PX; ++px) row[px][i] = fma(mij, d[px][j], row[px][i]);
-        }
-    }
+        for (int i = 0; i < N; ++i) Ns[px][i] = sm.base[i][px * FO_THREADS + tid] + (int32_t)((win[px] >> (N - 1 - i)) & 1u);
 #pragma unroll
     for (int px = 0; px < FO_PX; ++px) {
-        double Ed = 0.0;
-#pragma unroll
-        for (int i = 0; i < N; ++i) Ed = fma(d[px][i], row[px][i], Ed);
         if (live[px]) {
-            outE[gp[px]] = 0.5 * Ed;
+            outE[gp[px]] = Ebase[px] + dE[px];
             if (ns == 0) {
                 if constexpr (N % 4 == 0) {
                     if ((reinterpret_cast<uintptr_t>(outN) & 15u) == 0) {
@@ -670,7 +666,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
                                                                             double *__restrict__ xcont, qa_stats *stats)
 {
     constexpr int PIX = FO_THREADS;
-    __shared__ __align__(16) FoSmem<N, true, PIX> sm;
+    __shared__ __align__(16) FoSmem<N, true, PIX, true> sm;
     __shared__ double sx[N][PIX];  // the continuous minimum x of every pixel slot, read again by every pass
     const int tid = threadIdx.x;
     const int64_t p = (int64_t)blockIdx.x * PIX + tid;
@@ -751,7 +747,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
         int32_t *__restrict__ outN = ma.N[a];
         double *__restrict__ outE = ma.E[a];
         // ---- S4 (Eq. (9), readings R4 / R10) and the base-point gradient
-        double hp[N];
+        double hp[N], Ebase, dE;  // E(N*) = E(base) + dE, as in qa_fused_open_kernel
         unsigned fm = 0;
         {
             double d0[N], grad[N];
@@ -771,6 +767,10 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
             }
 #pragma unroll
             for (int b = 0; b < N; ++b) hp[b] = grad[N - 1 - b] + 0.5 * sm.MT[(N - 1 - b) * N + (N - 1 - b)];
+            double eb = 0.0;
+#pragma unroll
+            for (int i = 0; i < N; ++i) eb = fma(d0[i], grad[i], eb);
+            Ebase = 0.5 * eb;
         }
         unsigned win = 0;
         asm volatile("" ::: "memory");
@@ -854,6 +854,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
                     }
                 }
                 win = bkey;
+                dE = best - (offw + offu);
             } else {
                 // counting-order walk over all 2^N patterns (qa_fused_open_kernel, plain form)
                 constexpr int LB = N < 4 ? N : 4;
@@ -897,6 +898,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
                         }
                     }
                 }
+                dE = m;
             }
         } else {
             // thresholded: compaction of the free dots, bucket sort of the CTA's pixels by k, walk, hand back
@@ -947,32 +949,21 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
                     }
                 }
                 sm.sort.wkey[slot] = (unsigned char)bkey;
+                sm.cs[0][slot] = best;
             }
             __syncthreads();
             win = sm.sort.wkey[tid];
+            dE = sm.cs[0][tid];
         }
         // (compiler barriers: without them the M values the gradient phase loaded are kept for the epilogue, in local memory)
         asm volatile("" ::: "memory");
-        // ---- S7: N* = base + bits of the winner; E(N*) = 1/2 d^T M d from the definition (Eq. (C1))
+        // ---- S7: N* = base + bits of the winner; E(N*) = E(base) + dE
         {
             int32_t Ns[N];
-            double d[N], row[N];
 #pragma unroll
-            for (int i = 0; i < N; ++i) {
-                Ns[i] = sm.base[i][tid] + (int32_t)((win >> (N - 1 - i)) & 1u);
-                d[i] = (double)Ns[i] - sm.nc[i][tid];
-                row[i] = 0.0;
-            }
-#pragma unroll
-            for (int j = 0; j < N; ++j) {
-#pragma unroll
-                for (int i = 0; i < N; ++i) row[i] = fma(sm.MT[j * N + i], d[j], row[i]);
-            }
-            double Ed = 0.0;
-#pragma unroll
-            for (int i = 0; i < N; ++i) Ed = fma(d[i], row[i], Ed);
+            for (int i = 0; i < N; ++i) Ns[i] = sm.base[i][tid] + (int32_t)((win >> (N - 1 - i)) & 1u);
             if (live) {
-                outE[gp] = 0.5 * Ed;
+                outE[gp] = Ebase + dE;
                 if (N % 4 == 0 && (reinterpret_cast<uintptr_t>(outN) & 15u) == 0) {
 #pragma unroll
                     for (int i = 0; i + 3 < N; i += 4)
