@@ -4,8 +4,8 @@
 // (BASELINE.json configs[4]: 256 arrays x 128x128 pixels x {default, t = 0.2, t = 0.5}); blockIdx.y selects the model.
 //
 // What bounds it: V_g is the only HBM read (8 g bytes per pixel), N*, E(N*) the only writes, so the
-// floor is HBM (104 B per pixel at n = g = 8); the arithmetic next to it is ~200 FP64 instructions of per-pixel prologue
-// and epilogue (N_c: n g FMA, M d0: n^2 FMA, E(N*) from the definition: n^2 + n FMA) plus the candidate walk.  Every FMA
+// floor is HBM (104 B per pixel at n = g = 8); the arithmetic next to it is ~140 FP64 instructions of per-pixel prologue
+// and epilogue (N_c: n g FMA, M d0: n^2 FMA, E(base): n FMA) plus the candidate walk.  Every FMA
 // of the prologue takes one operand from a per-MODEL matrix, i.e. a warp-uniform value that has to come out of shared
 // memory (the model differs per CTA, so the constant bank is not available).  The kernel is a template over PX = pixels
 // per thread.  PX = 2 halves that operand traffic (every uniform operand serves two FMAs / DADDs) but needs 128 registers
@@ -29,7 +29,10 @@
 //                 free bits below it, so the linear part moves by c_j = h_{f_j} - sum_{i<j} h_{f_i} (stored per pixel in
 //                 shared memory, read with a warp-uniform j) and the bit pattern by an XOR mask; ascending st is ascending
 //                 pattern, so the strict '<' keeps the lexicographically smallest N among equal energies (reading R6).
-//   The winner's energy E(N*) is recomputed from the definition (Eq. (C1)) by the thread that owns the pixel.
+//   The winner's energy is E(N*) = E(base) + dE: E(base) = 1/2 d0^T M d0 from the definition (Eq. (C1); the gradient
+//   M d0 is already there) and dE = sum_{i in b} h_i + pairs(b), the increment the walk has minimised (the same expansion of
+//   (C1) around the base point).  Round 2 recomputed the whole quadratic form for N* instead (n^2 + n more FMAs and N_c parked
+//   in shared memory): 10 % of the kernel for the same result to a few ulp of E_C.
 #include "qa_internal.cuh"
 #include "qa_prologue.cuh"
 
