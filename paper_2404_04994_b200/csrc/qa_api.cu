@@ -174,6 +174,19 @@ qa_status rebuild(qa_model *m)
             h.QHT[t] = q;
         }
     }
+    if (n <= 8) {  // staging block of the one-kernel path (layout: QaDevModel::fo_pack)
+        double *pk = h.fo_pack;
+        for (int j = 0; j < n; ++j)
+            for (int i = 0; i < n; ++i) pk[j * n + i] = h.M[i * QA_MAXN + j];
+        pk += n * n;
+        for (int i = 0; i < n; ++i)
+            for (int j = 0; j < n; ++j) pk[i * n + j] = h.C[i * QA_MAXN + j];
+        pk += n * n;
+        for (int b = 0; b < (1 << n); ++b) pk[b] = h.QL[b];
+        pk += 1 << n;
+        for (int k = 0; k < m->g; ++k)
+            for (int i = 0; i < n; ++i) pk[k * n + i] = h.Cgd[i * QA_MAXG + k];
+    }
     // The source is pageable and the kernels run on non-blocking streams, which are not ordered against the legacy
     // stream: wait until the copy has landed and nothing else on the device can still read the old constants.
     QA_CUDA(cudaMemcpy(m->dev, &h, sizeof(h), cudaMemcpyHostToDevice));

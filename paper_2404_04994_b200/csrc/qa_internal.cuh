@@ -41,6 +41,10 @@ struct QaDevModel {
     double VT[(1 << QA_WALK_NL) * QA_WALK_NL];
     double QHT[1 << QA_WALK_NL];
     double VTt[QA_WALK_NL * (1 << QA_WALK_NL)];  // VT transposed, [j][t]: coalesced when the lanes hold consecutive t
+    // One-kernel path of n <= 8 (qa_kernels_fused_open.cu): its shared-memory tables as ONE contiguous block, so that a CTA
+    // stages them with 16-byte copies and no index arithmetic:  MT[j*n + i] = M[i][j] (n^2) | C compact row-major (n^2) |
+    // T[b] = QL[b] (2^n) | CgT[k*n + i] = Cgd[i][k] (g n, zero padded to an even count).  Zero for n > 8.
+    alignas(16) double fo_pack[2 * 64 + 256 + QA_MAXG * 8 + 2];
 };
 
 // Per-call scratch, structure-of-arrays over pixels ([i][P] so that thread-per-pixel accesses coalesce).

@@ -98,6 +98,21 @@ __device__ __forceinline__ int fo_qp_open(const double *__restrict__ sC, const d
     return rounds;
 }
 
+// The model's tables into shared memory: QaDevModel::fo_pack holds MT | C | T (contiguous in FoSmem as well) and CgT in the
+// kernel's layout, so the CTA copies 16 bytes per thread and step, without index arithmetic.
+template <int N>
+__device__ __forceinline__ void fo_stage(const QaDevModel *__restrict__ mdl, int g, int tid, double *sMT_C_T, double *sCgT)
+{
+    constexpr int N1 = (2 * N * N + (1 << N)) / 2;  // double2 entries of MT | C | T (an even number of doubles)
+    static_assert((2 * N * N + (1 << N)) % 2 == 0, "16-byte copies");
+    const double2 *__restrict__ src = reinterpret_cast<const double2 *>(mdl->fo_pack);
+    double2 *dst = reinterpret_cast<double2 *>(sMT_C_T);
+    for (int e = tid; e < N1; e += FO_THREADS) dst[e] = __ldg(src + e);
+    const int n2 = (g * N + 1) >> 1;  // C_gd^T, zero padded to an even count (both sides have the room)
+    double2 *dst2 = reinterpret_cast<double2 *>(sCgT);
+    for (int e = tid; e < n2; e += FO_THREADS) dst2[e] = __ldg(src + N1 + e);
+}
+
 template <int N, bool THR, int PIX>
 struct FoSort {  // thresholded: bookkeeping of the bucket sort and the walk
     unsigned long long xm[THR ? PIX : 1];  // XOR masks of the steps, 8 bits per free dot
@@ -116,7 +131,7 @@ struct FoSmem {
     double cs[THR ? N : 1][PIX];     // thresholded: c_j of the compacted free dots, per pixel slot
     int bucket[16];                  // thresholded: pixels of the CTA per number of free dots (outside the union below:
                                      // zeroed before the first barrier)
-    union {                    // C_gd is dead after S1 (a barrier separates it from the sort's first write)
+    union alignas(16) {        // C_gd is dead after S1 (a barrier separates it from the sort's first write)
         double CgT[QA_MAXG * N];   // CgT[k*N + i] = C_gd[i][k]
         FoSort<N, THR, PIX> sort;
     };
@@ -264,12 +279,7 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
     double va[FO_PX][8];
     load_chunk(0, va);
     const QaDevModel *__restrict__ mdl = models[blockIdx.y];
-    for (int e = tid; e < N * N; e += FO_THREADS) {
-        sm.MT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
-        sm.C[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
-    }
-    for (int e = tid; e < N * g; e += FO_THREADS) sm.CgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
-    for (int k = tid; k < (1 << N); k += FO_THREADS) sm.T[k] = mdl->QL[k];
+    fo_stage<N>(mdl, g, tid, sm.MT, sm.CgT);
     if (THR && tid < 16) sm.bucket[tid] = 0;
     const int ns = mdl->ns;
     const double EC = MP ? mdl->EC : 0.0;
@@ -693,12 +703,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
     double va[8];
     load_chunk(0, va);
     const QaDevModel *__restrict__ mdl = models[blockIdx.y];
-    for (int e = tid; e < N * N; e += FO_THREADS) {
-        sm.MT[e] = mdl->M[(e % N) * QA_MAXN + (e / N)];
-        sm.C[e] = mdl->C[(e / N) * QA_MAXN + (e % N)];
-    }
-    for (int e = tid; e < N * g; e += FO_THREADS) sm.CgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
-    for (int k = tid; k < (1 << N); k += FO_THREADS) sm.T[k] = mdl->QL[k];
+    fo_stage<N>(mdl, g, tid, sm.MT, sm.CgT);
     const double EC = MP ? mdl->EC : 0.0;
     __syncthreads();
 
