@@ -43,6 +43,7 @@ constexpr int FO_THREADS = 128;
 // batches are in flight before their DADDs (measured, config 5 default pass: 0.412 -> 0.399 ms)
 constexpr int FO_MP_CTAS = 6;
 constexpr int FO_MULTI_CTAS = 6;
+constexpr double FO_NOSORT_T = 0.6;  // thresholded: at or below this t the pixels are not bucket-sorted (measured on config 5: crossover between 0.5 and 0.7)
 constexpr int FO_PX_RUN = 1;  // pixels per thread the launcher instantiates (measured, config 5: 1.21 ms per step vs 1.49 with 2)
 // PX = pixels per thread (2: every uniform operand serves two FMAs; 1: half the registers and shared memory per CTA, twice
 // the CTAs per SM -- the thresholded kernels are bound by latency, not by the FP64 pipe), PIX = FO_THREADS * PX per CTA
@@ -531,6 +532,42 @@ __global__ void __launch_bounds__(FO_THREADS, MP ? FO_MP_CTAS : 4 * (3 - PX)) qa
         }
 #pragma unroll
         for (int px = 0; px < FO_PX; ++px) dE[px] = m[px];
+    } else if (args.t <= FO_NOSORT_T) {
+        // small thresholds (few free dots per pixel: 2^k = 4.3 candidates on average at t = 0.2, rarely more than 16): every
+        // thread walks its own pixels; the warp runs at the pace of its largest set, but there is no sort and no CTA barrier
+#pragma unroll
+        for (int px = 0; px < FO_PX; ++px) {
+            const int slot = px * FO_THREADS + tid;
+            double pre = 0.0;
+            int jj = 0;
+            unsigned low = 0;
+            unsigned long long xm = 0;
+#pragma unroll
+            for (int b = 0; b < N; ++b) {
+                if ((freem[px] >> b) & 1u) {
+                    sm.cs[jj][slot] = hp[px][b] - pre;
+                    pre += hp[px][b];
+                    xm |= (unsigned long long)((1u << b) | low) << (8 * jj);
+                    low |= 1u << b;
+                    ++jj;
+                }
+            }
+            const unsigned nst = live[px] ? 1u << jj : 1u;
+            double s = 0.0, best = 0.0;
+            unsigned key = 0, bkey = 0;
+            for (unsigned st = 1; st < nst; ++st) {
+                const int j = __ffs(st) - 1;
+                s += sm.cs[j][slot];
+                key ^= (unsigned)(xm >> (8 * j)) & 0xffu;
+                const double e = s + sm.T[key];
+                if (e < best) {
+                    best = e;
+                    bkey = key;
+                }
+            }
+            win[px] = bkey;
+            dE[px] = best;
+        }
     } else {
         // compaction of the free dots (ascending bit position), bucket sort of the CTA's pixels by k, walk, hand back
         __syncthreads();  // every warp is done with C_gd: its storage becomes the sort's
