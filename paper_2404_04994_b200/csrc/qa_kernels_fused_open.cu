@@ -22,8 +22,10 @@
 //   default:      the static counting-order walk of qa_kernels_walk.cu over all 2^n patterns, the thread's PX pixels at once
 //                 (3 FP64 instructions per candidate and pixel, one table entry per candidate for all of them).
 //   thresholded:  the number of free dots k differs from pixel to pixel (2^k candidates: 4.3 on average at t = 0.2, 25.6
-//                 at t = 0.5, but up to 256), so a warp of neighbouring pixels would run at the pace of its largest set.  The
-//                 pixels of a CTA are therefore bucket-sorted by k in shared memory and every thread walks PX
+//                 at t = 0.5, but up to 256), so a warp of neighbouring pixels runs at the pace of its largest set.  For
+//                 t <= FO_NOSORT_T = 0.6 that is accepted (every thread walks its own pixels: no sort, no CTA barrier;
+//                 measured faster on config 5 up to t ~ 0.6); above, the
+//                 pixels of a CTA are bucket-sorted by k in shared memory and every thread walks PX
 //                 pixels of (nearly) equal k.  The walk is the counting-order walk restricted to the free dots: with the
 //                 free dots f_0 < f_1 < .. (bit positions) the step st-1 -> st sets free bit j = ctz(st) and clears the
 //                 free bits below it, so the linear part moves by c_j = h_{f_j} - sum_{i<j} h_{f_i} (stored per pixel in
