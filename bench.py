@@ -451,7 +451,7 @@ def run_config5(args, rank, world, local_rank, steps=None, emit=True):
             "agreement_with_default": agree,
             "one_launch": {"ms_per_step": ms_multi, "pixels_per_s": world * px_step / (ms_multi * 1e-3),
                            "api": "qa_ground_state_batch_multi: the three algorithms in ONE launch (V_g, N_c and the QP once per "
-                                  "pixel; results bit-identical; 17 % fewer instructions, but measured slower on B200: DESIGN.md 5.5)",
+                                  "pixel; results bit-identical; measured 5 % slower than three launches on B200: DESIGN.md 5.5)",
                            "algorithmic_bytes_per_step": B * P * (8 * g + len(algs) * (4 * n + 8))},
             "roofline": {"bound": "hbm", "kernel": "qa_fused_open_kernel (whole step: 3 launches)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,

@@ -740,8 +740,19 @@ qa_status qa_ground_state_batch_multi(const qa_batch *bt, const double *d_Vg, in
     }
     if (P == 0) return QA_OK;
     if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
-    QA_CUDA(qa_launch_fused_open_multi(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, bt->general, ma, d_xcont, d_stats,
-                                       static_cast<cudaStream_t>(cuda_stream)));
+    bool one_launch = true;  // the one-launch kernel has the sort-free thresholded walk only
+    for (int a = 0; a < n_alg; ++a)
+        if (ma.thr[a] && ma.t[a] > QA_FO_NOSORT_T) one_launch = false;
+    if (one_launch) {
+        QA_CUDA(qa_launch_fused_open_multi(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, bt->general, ma, d_xcont,
+                                           d_stats, static_cast<cudaStream_t>(cuda_stream)));
+        return QA_OK;
+    }
+    for (int a = 0; a < n_alg; ++a) {  // a large threshold among them: one launch per algorithm, same results
+        QaCallArgs ca{0, 0, ma.thr[a] ? (int)QA_ALG_THRESHOLDED : (int)QA_ALG_DEFAULT, ma.t[a], 0, bt->general};
+        QA_CUDA(qa_launch_fused_open(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, ca, ma.N[a], ma.E[a], d_xcont, nullptr,
+                                     d_stats, static_cast<cudaStream_t>(cuda_stream)));
+    }
     return QA_OK;
 }
 

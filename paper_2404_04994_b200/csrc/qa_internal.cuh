@@ -73,6 +73,9 @@ struct QaCallArgs {
 
 // Several algorithms on one sweep in one launch (qa_ground_state_batch_multi): per pass the threshold and the outputs.
 constexpr int QA_MULTI_MAX = 4;
+// thresholded algorithm in the one-kernel path of n <= 8: at or below this t the pixels are not bucket-sorted by their number
+// of free dots (measured on config 5: crossover between 0.5 and 0.7); the multi-algorithm kernel has only that form
+constexpr double QA_FO_NOSORT_T = 0.6;
 struct QaMultiArgs {
     int n_alg;
     int thr[QA_MULTI_MAX];      // 1: thresholded (Eq. (9)), 0: default

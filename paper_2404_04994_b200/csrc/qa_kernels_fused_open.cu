@@ -44,8 +44,8 @@ constexpr int FO_THREADS = 128;
 // CTAs per SM the min-plus default walk is compiled for: 80 registers instead of 64, so that the table reads of several
 // batches are in flight before their DADDs (measured, config 5 default pass: 0.412 -> 0.399 ms)
 constexpr int FO_MP_CTAS = 6;
-constexpr int FO_MULTI_CTAS = 6;
-constexpr double FO_NOSORT_T = 0.6;  // thresholded: at or below this t the pixels are not bucket-sorted (measured on config 5: crossover between 0.5 and 0.7)
+constexpr int FO_MULTI_CTAS = 8;
+constexpr double FO_NOSORT_T = QA_FO_NOSORT_T;  // thresholded: at or below this t the pixels are not bucket-sorted (measured on config 5: crossover between 0.5 and 0.7)
 constexpr int FO_PX_RUN = 1;  // pixels per thread the launcher instantiates (measured, config 5: 1.21 ms per step vs 1.49 with 2)
 // PX = pixels per thread (2: every uniform operand serves two FMAs; 1: half the registers and shared memory per CTA, twice
 // the CTAs per SM -- the thresholded kernels are bound by latency, not by the FP64 pipe), PIX = FO_THREADS * PX per CTA
@@ -718,8 +718,19 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
                                                                             double *__restrict__ xcont, qa_stats *stats)
 {
     constexpr int PIX = FO_THREADS;
-    __shared__ __align__(16) FoSmem<N, true, PIX, true> sm;
-    __shared__ double sx[N][PIX];  // the continuous minimum x of every pixel slot, read again by every pass
+    // 27 KB at N = 8: eight CTAs per SM.  N_c and x of every pixel slot wait here for every pass; the base point is not
+    // parked (the epilogue recomputes floor(x) and keeps one bit per dot for "rounded up")
+    struct Smem {
+        double MT[N * N], C[N * N], T[1 << N];  // contiguous: fo_stage
+        double nc[N][PIX];
+        double x[N][PIX];
+        union alignas(16) {
+            double CgT[QA_MAXG * N];  // dead after S1
+            double cs[N][PIX];        // thresholded passes: c_j of the compacted free dots of the thread's own pixel
+        };
+    };
+    __shared__ __align__(16) Smem sm;
+    double(*sx)[PIX] = sm.x;
     const int tid = threadIdx.x;
     const int64_t p = (int64_t)blockIdx.x * PIX + tid;
     const bool live = p < P;
@@ -785,7 +796,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
     }
 #pragma unroll
     for (int i = 0; i < N; ++i) sx[i][tid] = x[i];
-    __syncthreads();  // every warp is done with C_gd: its storage becomes the sort's (thresholded passes)
+    __syncthreads();  // every warp is done with C_gd: its storage becomes the c_j columns of the thresholded passes
 
 #pragma unroll 1
     for (int a = 0; a < ma.n_alg; ++a) {
@@ -795,16 +806,19 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
         double *__restrict__ outE = ma.E[a];
         // ---- S4 (Eq. (9), readings R4 / R10) and the base-point gradient
         double hp[N], Ebase, dE;  // E(N*) = E(base) + dE, as in qa_fused_open_kernel
-        unsigned fm = 0;
+        unsigned fm = 0, up = 0;
         {
             double d0[N], grad[N];
 #pragma unroll
             for (int i = 0; i < N; ++i) {
                 int32_t cn, bs;
-                qa_floor_ceil(sx[i][tid], tt, thr, bs, cn);
+                const double xi = sx[i][tid];
+                qa_floor_ceil(xi, tt, thr, bs, cn);
                 if (cn == 2) fm |= 1u << (N - 1 - i);
+                const double fl = floor(xi);
+                const int32_t lo = fl > 0.0 ? (int32_t)fl : 0;
+                up |= (unsigned)(bs - lo) << (N - 1 - i);  // 1: the base point is lo + 1 (thresholded, fraction >= 1/2)
                 d0[i] = (double)bs - sm.nc[i][tid];
-                sm.base[i][tid] = bs;
                 grad[i] = 0.0;
             }
 #pragma unroll
@@ -948,59 +962,36 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
                 dE = m;
             }
         } else {
-            // thresholded: compaction of the free dots, bucket sort of the CTA's pixels by k, walk, hand back
-            if (tid < 16) sm.bucket[tid] = 0;
-            __syncthreads();
-            {
-                double pre = 0.0;
-                int jj = 0;
-                unsigned low = 0;
-                unsigned long long xm = 0;
+            // thresholded (the launcher admits t <= QA_FO_NOSORT_T only): every thread walks its own pixel, no sort, no barrier
+            double pre = 0.0;
+            int jj = 0;
+            unsigned low = 0;
+            unsigned long long xm = 0;
 #pragma unroll
-                for (int b = 0; b < N; ++b) {
-                    if ((fm >> b) & 1u) {
-                        sm.cs[jj][tid] = hp[b] - pre;
-                        pre += hp[b];
-                        xm |= (unsigned long long)((1u << b) | low) << (8 * jj);
-                        low |= 1u << b;
-                        ++jj;
-                    }
+            for (int b = 0; b < N; ++b) {
+                if ((fm >> b) & 1u) {
+                    sm.cs[jj][tid] = hp[b] - pre;
+                    pre += hp[b];
+                    xm |= (unsigned long long)((1u << b) | low) << (8 * jj);
+                    low |= 1u << b;
+                    ++jj;
                 }
-                const int kf = live ? jj : 0;
-                sm.sort.xm[tid] = xm;
-                sm.sort.kfree[tid] = (unsigned char)kf;
-                sm.sort.wkey[tid] = 0;
-                const int rk = fo_bucket_rank(sm.bucket, N - kf);
-                __syncthreads();
-                int start = 0;
-#pragma unroll
-                for (int bkt = 0; bkt <= N; ++bkt)
-                    if (bkt < N - kf) start += sm.bucket[bkt];
-                sm.sort.order[start + rk] = (unsigned short)tid;
             }
-            __syncthreads();
-            {
-                const int slot = sm.sort.order[tid];
-                const unsigned nst = 1u << sm.sort.kfree[slot];
-                const unsigned long long xm = sm.sort.xm[slot];
-                double sl = 0.0, best = 0.0;
-                unsigned key = 0, bkey = 0;
-                for (unsigned st = 1; st < nst; ++st) {
-                    const int j = __ffs(st) - 1;
-                    sl += sm.cs[j][slot];
-                    key ^= (unsigned)(xm >> (8 * j)) & 0xffu;
-                    const double e = sl + sm.T[key];
-                    if (e < best) {
-                        best = e;
-                        bkey = key;
-                    }
+            const unsigned nst = live ? 1u << jj : 1u;
+            double sl = 0.0, best = 0.0;
+            unsigned key = 0, bkey = 0;
+            for (unsigned st = 1; st < nst; ++st) {
+                const int j = __ffs(st) - 1;
+                sl += sm.cs[j][tid];
+                key ^= (unsigned)(xm >> (8 * j)) & 0xffu;
+                const double e = sl + sm.T[key];
+                if (e < best) {
+                    best = e;
+                    bkey = key;
                 }
-                sm.sort.wkey[slot] = (unsigned char)bkey;
-                sm.cs[0][slot] = best;
             }
-            __syncthreads();
-            win = sm.sort.wkey[tid];
-            dE = sm.cs[0][tid];
+            win = bkey;
+            dE = best;
         }
         // (compiler barriers: without them the M values the gradient phase loaded are kept for the epilogue, in local memory)
         asm volatile("" ::: "memory");
@@ -1008,7 +999,11 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
         {
             int32_t Ns[N];
 #pragma unroll
-            for (int i = 0; i < N; ++i) Ns[i] = sm.base[i][tid] + (int32_t)((win >> (N - 1 - i)) & 1u);
+            for (int i = 0; i < N; ++i) {
+                const double fl = floor(sx[i][tid]);
+                const int32_t lo = fl > 0.0 ? (int32_t)fl : 0;
+                Ns[i] = lo + (int32_t)((up >> (N - 1 - i)) & 1u) + (int32_t)((win >> (N - 1 - i)) & 1u);
+            }
             if (live) {
                 outE[gp] = Ebase + dE;
                 if (N % 4 == 0 && (reinterpret_cast<uintptr_t>(outN) & 15u) == 0) {

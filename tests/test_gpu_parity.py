@@ -502,6 +502,11 @@ def test_batch_multi_equals_separate_calls(api, n):
         okw = dict(algorithm=name) if t is None else dict(algorithm=name, t=t)
         o = om.ground_state(wls[1].Vg, **okw)
         compare(rm[k]["N"][1].cpu().numpy(), rm[k]["E"][1].cpu().numpy(), o, om.EC, gpu_x=rm[0]["xcont"][1].cpu().numpy())
+    # a threshold above 0.6 among them: the call falls back to one launch per algorithm, same results
+    rf = batch.ground_state_multi(Vg, [("thresholded", 0.8), ("default", None)])
+    assert api.last_launch_plan()[0] == ["qa_fused_open_kernel", "qa_fused_open_kernel"]
+    r8 = batch.ground_state(Vg, algorithm="thresholded", t=0.8)
+    assert torch.equal(rf[0]["N"], r8["N"]) and torch.equal(rf[0]["E"], r8["E"]) and torch.equal(rf[1]["N"], rm[1]["N"])
     with pytest.raises(api.QaError):
         batch.ground_state_multi(Vg, [("brute", None)])
     with pytest.raises(api.QaError):
