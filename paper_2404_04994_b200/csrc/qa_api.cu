@@ -174,6 +174,9 @@ qa_status rebuild(qa_model *m)
             h.QHT[t] = q;
         }
     }
+    h.qsum = 0.0;
+    for (int i = 0; i < n; ++i)
+        for (int j = i + 1; j < n; ++j) h.qsum += std::fabs(h.M[i * QA_MAXN + j]);
     if (n <= 8) {  // staging block of the one-kernel path (layout: QaDevModel::fo_pack)
         double *pk = h.fo_pack;
         for (int j = 0; j < n; ++j)
@@ -243,6 +246,8 @@ size_t carve(const qa_model *m, int64_t P, void *base, QaWorkspace *ws)
         ws->e0 = e0;
         ws->rec = rec;
         ws->rec2 = reinterpret_cast<double2 *>(rec);
+        // n >= 13: the walk's records take 8 * 2^(n-13) <= 64 bytes per pixel of the 256 the region has
+        ws->ext = n >= 13 ? reinterpret_cast<double *>(reinterpret_cast<char *>(rec) + Pz * 64) : nullptr;
         ws->counter = counter;
         ws->P = P;
     }
@@ -273,7 +278,9 @@ qa_status ground_state(const qa_model *m, const double *d_Vg, int64_t P, int clo
     QaWorkspace ws;
     carve(m, P, d_ws, &ws);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1};
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1, 0};
+    // the min-plus walk follows the prologue: have it write the walk's per-pixel constants as well (ws.ext)
+    if (alg == QA_ALG_DEFAULT && !closed && n >= 13 && variant == 1 && m->is_z) a.walk_ext = 1;
     g_n_marks = 0;
     timing_mark(stream);
     // small arrays with small candidate sets: the whole path in one kernel, one thread per pixel (no workspace traffic)
@@ -366,7 +373,7 @@ qa_status thermal(const qa_model *m, const double *d_Vg, int64_t P, int closed, 
     QaWorkspace ws;
     carve(m, P, d_ws, &ws);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1};
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, m->is_z ? 0 : 1, 0};
     g_n_marks = 0;
     timing_mark(stream);
     QA_CUDA(qa_launch_prologue(m->dev, n, m->g, d_Vg, ws, a, nullptr, d_stats, stream,
@@ -709,7 +716,7 @@ qa_status qa_ground_state_batch(const qa_batch *bt, const double *d_Vg, int64_t 
     }
     if (P == 0) return QA_OK;
     if (P > (int64_t)1 << 40) return QA_ERR_INVALID_ARG;
-    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, bt->general};
+    QaCallArgs a{closed, N_hat, (int)alg, t, n_max, bt->general, 0};
     if (!closed && alg != QA_ALG_BRUTE_FORCE)
         QA_CUDA(qa_launch_fused_open(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, a, d_N, d_E, d_xcont, nullptr, d_stats,
                                      static_cast<cudaStream_t>(cuda_stream)));
@@ -749,7 +756,7 @@ qa_status qa_ground_state_batch_multi(const qa_batch *bt, const double *d_Vg, in
         return QA_OK;
     }
     for (int a = 0; a < n_alg; ++a) {  // a large threshold among them: one launch per algorithm, same results
-        QaCallArgs ca{0, 0, ma.thr[a] ? (int)QA_ALG_THRESHOLDED : (int)QA_ALG_DEFAULT, ma.t[a], 0, bt->general};
+        QaCallArgs ca{0, 0, ma.thr[a] ? (int)QA_ALG_THRESHOLDED : (int)QA_ALG_DEFAULT, ma.t[a], 0, bt->general, 0};
         QA_CUDA(qa_launch_fused_open(bt->dev_list, bt->n_models, bt->n, bt->g, d_Vg, P, ca, ma.N[a], ma.E[a], d_xcont, nullptr,
                                      d_stats, static_cast<cudaStream_t>(cuda_stream)));
     }

@@ -27,6 +27,8 @@ struct QaDevModel {
     double C1[QA_MAXN];             // c_dd 1        (Eq. (7))
     double oneC1;                   // 1^T c_dd 1
     double EC;                      // 1/2 min_i M_ii
+    double qsum;                    // sum_{i<j} |M_ij| of the search model (>= the pair energy of any bit pattern)
+    double pad16;                   // (keeps the 16-byte alignment of the tables below: they are read as double2)
     double Mf[QA_MAXN * QA_MAXN];   // full c_dd^-1, stride QA_MAXN
     double Cgdf[QA_MAXN * QA_MAXG]; // full c_gd
     int arr_idx[QA_MAXN];           // search dot a -> dot index in the full model
@@ -59,6 +61,10 @@ struct QaWorkspace {
     unsigned long long *counter;  // work counter of the pruned min-plus walk (zeroed by the prologue kernel)
     uint2 *rec;       // [P][2^(n-13)]  min-plus walk: per warp of the pixel (min of L over its lanes, ballot of lanes near it)
     double2 *rec2;    // [nb][P]        closed walk (same storage as rec): per block of high patterns (best energy, its index)
+    // [3][P] (n >= 13, behind the walk's records in the same region): thread-independent per-pixel constants of the min-plus
+    // walk, written by the lanes prologue: offW = E_C + sum |h| of the 4 lowest bits' dots, offU = sum |h| of the next 4,
+    // C' = the fixed-point constant of the keys (qa_kernels_minplus.cu)
+    double *ext;
     int64_t P;
 };
 
@@ -69,6 +75,7 @@ struct QaCallArgs {
     double t;
     int n_max;
     int general_qp;  // c_dd has a positive off-diagonal: the QP continues with the primal active-set phase (R3)
+    int walk_ext;    // 1: the min-plus walk follows (open, default, n >= 13, Maxwell): the lanes prologue also writes ws.ext
 };
 
 // Several algorithms on one sweep in one launch (qa_ground_state_batch_multi): per pass the threshold and the outputs.

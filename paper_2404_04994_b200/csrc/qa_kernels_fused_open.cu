@@ -1021,7 +1021,7 @@ __global__ void __launch_bounds__(FO_THREADS, FO_MULTI_CTAS) qa_fused_open_multi
         bool failed = failed0;
         if (live && slowf) {  // deferred pixel (see fo_slow_pixel): redone from scratch with this pass's algorithm
             int st3[3];
-            QaCallArgs sa{0, 0, thr ? (int)QA_ALG_THRESHOLDED : (int)QA_ALG_DEFAULT, tt, 0, general_qp};
+            QaCallArgs sa{0, 0, thr ? (int)QA_ALG_THRESHOLDED : (int)QA_ALG_DEFAULT, tt, 0, general_qp, 0};
             if (thr)
                 fo_slow_pixel<N, true>(sm.MT, sm.C, sm.T, mdl, Vg, gp, sa, outN, outE, xcont, nullptr, st3);
             else

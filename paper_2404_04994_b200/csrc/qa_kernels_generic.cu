@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel
     for (int e = tid; e < N * g; e += 256) sCgT[e] = mdl->Cgd[(e % N) * QA_MAXG + (e / N)];
     if (tid < N) sC1[tid] = mdl->C1[tid];
     const double oneC1 = mdl->oneC1;
+    const double ECm = mdl->EC, QSm = mdl->qsum;  // (read up front: their latency hides behind the staging)
     const int64_t P = ws.P;
     const int64_t p0 = (int64_t)blockIdx.x * PPB;
     for (int e = tid; e < PPB * g; e += 256) {
@@ -150,6 +151,34 @@ __global__ void __launch_bounds__(256) qa_prologue_lanes_kernel(const QaDevModel
     if (live && i == 0) {
         ws.total[p] = total;
         ws.e0[p] = 0.5 * e0;
+    }
+    if constexpr (N >= 13) {
+        if (args.walk_ext) {
+            // Thread-independent per-pixel constants of the min-plus walk (qa_kernels_minplus.cu; low bit j <-> dot N-1-j, w =
+            // bits [0,4), u = bits [4,8)): offW = E_C + sum_{w dots} |h|, offU = sum_{u dots} |h|, and the fixed-point
+            // constant C' of the keys from a bound of A + y over the pixel:
+            //     A <= E(base) + E_C + QSUM + sum_high |h| + 2 sum_u |h| + 4 QSUM,   y <= E_C + 2 sum_w |h| + 5 QSUM,
+            // QSUM = the sum of all pair energies M_ij, i < j (QaDevModel::qsum).  bound < 2^(eb - 1022); one unit = 2^(eb - 1053), so that
+            // A + y < 2^31 units.
+            const double ah = dot ? fabs(gi + 0.5 * sMT[i * N + i]) : 0.0;
+            double sw = (dot && i >= N - 4) ? ah : 0.0;
+            double su = (dot && i >= N - 8 && i < N - 4) ? ah : 0.0;
+            double sh = (dot && i < N - 8) ? ah : 0.0;
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) {
+                sw += __shfl_xor_sync(0xffffffffu, sw, o);
+                su += __shfl_xor_sync(0xffffffffu, su, o);
+                sh += __shfl_xor_sync(0xffffffffu, sh, o);
+            }
+            const double offw = ECm + sw;
+            const double bound = fabs(0.5 * e0) + 2.0 * ((offw + su) + sh) + 10.0 * QSm;
+            const int eb = (__double2hiint(bound) >> 20) & 0x7ff;
+            if (live && i == 0) {
+                ws.ext[p] = offw;
+                ws.ext[P + p] = su;
+                ws.ext[2 * P + p] = __hiloint2double(((eb + 22) << 20) | 0x80000, 0);
+            }
+        }
     }
     __syncthreads();
     {   // coalesced stores: thread (row r, column c) of the [N][PPB] tiles

@@ -46,7 +46,9 @@
 //     definition (S7), so the path is three launches: prologue, walk, finish.
 //
 // FP64-pipe instructions per (thread, pixel) at NU = NW = 4, NH = 8: 256 (y) + 20 (A) + 16 (LB) + 15 (B) + 8 (h') + 8
-// (offsets) + 11 (be, a0, lo3) = 334 per 256 candidates, i.e. 1.30 per candidate (exact-compare Gray walk: 3).
+// (offsets) + 11 (be, a0, lo3) = 334 per 256 candidates, i.e. 1.30 per candidate (exact-compare Gray walk: 3).  With the
+// fixed-point keys (no LB additions) and offW, offU, C' read from ws.ext (written once per pixel by the lanes prologue,
+// qa_kernels_generic.cu) qa_minplus_walk_kernel needs 312 = 1.22 per candidate.
 //
 // Index convention as in qa_kernels_walk.cu: candidate index = sum_i b_i 2^(n-1-i) = (t << NL) | (u << NW) | w.
 #include "qa_internal.cuh"
@@ -214,7 +216,7 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
     constexpr int TPP = 1 << NH;             // threads per pixel
     constexpr int WPP = TPP / 32;            // warps per pixel
     constexpr int SLOTS = MP_THREADS / TPP;  // pixel groups in flight per CTA
-    constexpr int NV = N + 1;                // per-pixel inputs: h[0..N-1], E(base)
+    constexpr int NV = N + 1 + (ENC_ ? 3 : 0);  // per-pixel inputs: h[0..N-1], E(base) (+ offW, offU, C' from ws.ext)
     constexpr int NCH = 1 << (NU - 2);       // chunks of 4 u each
     static_assert(NH >= 5 && NH <= 8 && N <= 31 && NW >= 2 && NU >= 2, "one or more whole warps per pixel");
 
@@ -230,15 +232,6 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
     for (int j = 0; j < NL; ++j) v[j] = mdl->VT[t * NL + j];
     const double EC = mdl->EC;
     const double QH = mdl->QHT[t];
-    // ENC: sum of ALL pair energies M_ij, i < j (>= the pair energy of any pattern: M >= 0) = pairs among the high bits +
-    // pairs among the low bits + every cross term
-    double QSUM = 0.0;
-    if (ENC) {
-        QSUM = (mdl->QHT[TPP - 1] - EC) + tab.q[(1 << NL) - 1];
-#pragma unroll
-        for (int j = 0; j < NL; ++j) QSUM += mdl->VT[(TPP - 1) * NL + j];
-    }
-
     // Every slot (the TPP threads of one pixel group) is an independent worker; consecutive workers sit in different
     // CTAs so that a ragged last round is spread over all SMs.
     const int64_t groups = (P + PX - 1) / PX;
@@ -250,7 +243,8 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
         if (grp < groups && lane < NV) {
             int64_t p = grp * PX + px;
             if (p >= P) p = P - 1;  // ragged last group: the last pixel is walked twice, stored once
-            r = lane < N ? __ldg(ws.h + (int64_t)lane * P + p) : __ldg(ws.e0 + p);
+            r = lane < N ? __ldg(ws.h + (int64_t)lane * P + p)
+                         : (lane == N ? __ldg(ws.e0 + p) : __ldg(ws.ext + (int64_t)(lane - N - 1) * P + p));
         }
         return r;
     };
@@ -277,34 +271,31 @@ __global__ void __launch_bounds__(MP_THREADS, MINB) qa_minplus_walk_kernel(const
                 const double hj = mp_shfl(myv, N - 1 - j);
                 if (j < NW) {
                     hw[j] = hj + v[j];
-                    offw += fabs(hj);
+                    if (!ENC) offw += fabs(hj);
                 } else {
                     hu[px][j - NW] = hj + v[j];
-                    offu += fabs(hj);
+                    if (!ENC) offu += fabs(hj);
                 }
             }
-            const double e0h = mp_shfl(myv, N);
-            double be = e0h + QH, sumhigh = 0.0;
+            double be = mp_shfl(myv, N) + QH;
 #pragma unroll
             for (int jh = 0; jh < NH; ++jh) {
                 const double hv = mp_shfl(myv, N - 1 - NL - jh);
                 if ((t >> jh) & 1u) be += hv;
-                if (ENC) sumhigh += fabs(hv);
+            }
+            if (ENC) {  // thread-independent constants of the pixel, computed once by the prologue (ws.ext)
+                offw = mp_shfl(myv, N + 1);
+                offu = mp_shfl(myv, N + 2);
+                Cenc[px] = mp_shfl(myv, N + 3);
+            } else {
+                Cenc[px] = 0.0;
             }
             a0[px] = be + offu;
             lo3[px] = hu[px][1] + hu[px][0];
             B[px][0] = offw;
             if (ENC) {
-                // Thread-independent bound of A[u] + y over the whole pixel:  A <= E(base) + QSUM + E_C + sum_high |h| +
-                // 2 sum_u |h| + NU QSUM,  y <= E_C + 2 sum_w |h| + (NW + 1) QSUM.  bound < 2^(ex + 1); one unit = 2^(ex - 30),
-                // so that A + y < 2^31 units and the integer sums below cannot wrap.
-                const double bound = fabs(e0h) + 2.0 * ((offw + offu) + sumhigh) + (double)(NL + 2) * QSUM;
-                const int eb = (__double2hiint(bound) >> 20) & 0x7ff;   // biased exponent of the bound
-                Cenc[px] = __hiloint2double(((eb + 22) << 20) | 0x80000, 0);
                 a0[px] += Cenc[px];     // (every A[u] of the chunk loop then carries C': one rounding to the grid per add)
                 B[px][0] += Cenc[px];
-            } else {
-                Cenc[px] = 0.0;
             }
 #pragma unroll
             for (int w = 1; w < (1 << NW); ++w) B[px][w] = B[px][w & (w - 1)] + hw[mp_ctz(w)];
