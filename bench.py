@@ -34,7 +34,7 @@ import numpy as np  # noqa: E402
 METRIC = "candidate configs scored/s (16 dots, default algorithm, open 4x4 grid, 100x100 pixels)"
 UNIT = "candidates/s"
 FP64_OPS_PER_CANDIDATE = 312.0 / 256.0   # FP64-pipe instructions per candidate of the min-plus walk
-WALK_DRAM_BYTES_NCU = 1392896           # dram__bytes_read + dram__bytes_write per launch, from the ncu capture named below
+WALK_DRAM_BYTES_NCU = 1632768           # dram__bytes_read + dram__bytes_write per launch, from the ncu capture named below
 WALK_DRAM_SOURCE = "profiles/r02_headline_ncu_full.md"
 THERMAL_FP64_OPS_PER_CANDIDATE = {"qa_thermal_sp_kernel": 3.0}  # 2 DFMA (rows, columns) + 1 DADD (lower bound of the E_min pass)
 FP64_LANES_PER_SM = 64         # 148 SMs x 64 FP64 lanes x SM clock
