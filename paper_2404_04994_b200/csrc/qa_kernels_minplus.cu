@@ -29,7 +29,9 @@
 //   so |L_t - min e_t| <= 5 units and the thread of the arg min (and of every tie) has L_t <= min L + 10; the kernel keeps
 //   the lanes within MP_ENC_SLACK = 16.  One unit is ~2^-30 of the bound (~4e-8 E_C on config 4; the high-word keys resolve
 //   2^-20 of the value), so pass 2 sees fewer survivors, and the row bound costs an integer add instead of a DADD.
-//   Measured: walk 87.4 -> 85.0 us, identical N and E on every test.
+//   Measured: walk 87.4 -> 85.0 us, identical N and E on every test.  offW, offU and C' are the same for the 256 threads of
+//   a pixel: the lanes prologue computes them once per pixel (ws.ext) and the walk reads them with the other inputs
+//   (85.0 -> 80.0 us).
 //   qa_minplus_walk_kernel (pass 1; a lower bound per thread; the high-word form):
 //       m_u  = min_w hi32(y)                               (ALU pipe, VIMNMX3)
 //       LB_u = A[u] + double(m_u, 0)   <= min_w e(t,u,w)   (truncation and rounding are monotone)
