@@ -49,6 +49,12 @@ struct QaDevModel {
     alignas(16) double fo_pack[2 * 64 + 256 + QA_MAXG * 8 + 2];
 };
 
+// (kernels read these tables 16 bytes at a time)
+static_assert(offsetof(QaDevModel, QL) % 16 == 0 && offsetof(QaDevModel, VT) % 16 == 0 && offsetof(QaDevModel, QHT) % 16 == 0 &&
+                  offsetof(QaDevModel, VTt) % 16 == 0 && offsetof(QaDevModel, fo_pack) % 16 == 0 &&
+                  offsetof(QaDevModel, M) % 16 == 0 && offsetof(QaDevModel, C) % 16 == 0,
+              "QaDevModel: tables read as double2 must stay 16-byte aligned");
+
 // Per-call scratch, structure-of-arrays over pixels ([i][P] so that thread-per-pixel accesses coalesce).
 struct QaWorkspace {
     double *h;        // [n][P]  g0_i + 1/2 M_ii at the base point: energy increment of raising dot i by one
