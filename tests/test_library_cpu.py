@@ -49,8 +49,14 @@ def test_sass_is_sm100a_only():
 def test_status_strings_and_host_side_validation_without_gpu():
     from paper_2404_04994_b200 import api
     lib = api.lib()
-    for s in range(9):
+    for s in range(10):
         assert len(lib.qa_status_string(s)) > 0
+    # the entry point with the library's own static workspace, and the multi-algorithm batch call: argument errors are
+    # found on the host, before any CUDA call
+    assert lib.qa_static_workspace_bytes() == 16 << 20
+    assert lib.qa_ground_state_open_static(None, None, 10, 0, 1.0, 0, None, None, None, None, None, None) == 1
+    assert b"model is NULL" in lib.qa_static_workspace_last_error()
+    assert lib.qa_ground_state_batch_multi(None, None, 10, 1, None, None, None, None, None, None, None) == 1
     h = C.c_void_p()
     bad = np.array([[1.0, 0.5], [0.1, 1.0]])
     assert lib.qa_model_create(bad.ctypes.data, np.eye(2).ctypes.data, 2, 2, C.byref(h)) == 2      # not symmetric
